@@ -1,0 +1,152 @@
+"""O-ADMM: the paper's iteration, step by step, in fp64 numpy (test infrastructure).
+
+PARITY UNPINNED by the paper (no printed iterate); see oracle/__init__.py for the pins used.
+
+Follows PAPER.md section II.B in the paper's order and notation, three-variable scaled form:
+    (6)  v  = S^-1 ( A (z1 - y1 - c/rho) - z2 + y2 ),   S = A A^T + I  (factorised once, :91, :100)
+    (7)  x1 = z1 - y1 - c/rho - A^T v ;   x2 = v + z2 - y2
+    (4b) z1 = clip(x1 + y1, l=0, u) ;     z2 = min(x2 + y2, b)
+    (4c) y1 = y1 + x1 - z1 ;              y2 = y2 + x2 - z2
+batched by stacking the per-plan vectors as columns (:96), one rho per column (:222).
+A, c, b, u are the PRECONDITIONED data (III.C, :183, :213; readings R9-R11):
+    D_i = 1 / N_class(i)            column scaling, x = D x_hat            (R10)
+    R_j = 1 / || row j of A D ||_2  row normalisation => diag(S) = 2       (:213, R9)
+    A_hat = R A D,  c_hat = D c,  b_hat = R b,  u_hat = u / D.
+Initial iterate: all zeros (R6).  Beam-on times: t = rho * R o y2 (:80); lambda = D o z1.
+
+Stopping rule (the paper fixes 3000 iterations and gives no criterion, :106, :240; reading R7,
+Boyd et al. section 3.3 on the scaled problem, per plan, tested every `check_every` iterations):
+    ||x - z+||_2 <= eps_abs*sqrt(N+n) + tol*max(||x||_2, ||z+||_2)   and
+    ||z+ - z||_2 <= eps_abs*sqrt(N+n) + tol*||y+||_2
+(norms over both blocks stacked).  A plan that meets it is frozen at that iterate.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+import scipy.linalg
+
+from .lp_model import class_arrays
+
+
+@dataclass
+class Preconditioned:
+    A_hat: np.ndarray      # [n, N]
+    c_hat: np.ndarray      # [N]
+    D: np.ndarray          # [N]
+    R: np.ndarray          # [n]
+    S: np.ndarray          # [n, n]
+    chol: tuple            # scipy cho_factor(S)
+    class_count: np.ndarray
+
+
+def precondition(phi, point_class, classes) -> Preconditioned:
+    phi = np.asarray(phi, dtype=np.float64)
+    pc, sense, thr = class_arrays(point_class, classes)
+    Nk = np.bincount(pc, minlength=len(classes)).astype(np.float64)
+    D = 1.0 / Nk[pc]
+    A = (phi * (sense / thr)[:, None]).T            # Eq. (12) with varphi = phi / D_alpha (:326)
+    AD = A * D[None, :]
+    norms = np.sqrt(np.sum(AD * AD, axis=1))
+    R = np.where(norms > 0, 1.0 / np.where(norms > 0, norms, 1.0), 1.0)
+    A_hat = AD * R[:, None]
+    c_hat = D * (-sense)                            # Eq. (11)
+    S = A_hat @ A_hat.T + np.eye(A_hat.shape[0])    # :91
+    chol = scipy.linalg.cho_factor(S, lower=True)
+    return Preconditioned(A_hat=A_hat, c_hat=c_hat, D=D, R=R, S=S, chol=chol, class_count=Nk)
+
+
+def plan_bounds(pre: Preconditioned, point_class, classes, weights, masks: Optional[np.ndarray] = None):
+    """u_hat [N, B] and b_hat [n, B] (Eq. 13, 15 scaled).  masks: [B, N] bool or None (:144)."""
+    pc = np.asarray(point_class).astype(np.int64)
+    weights = np.asarray(weights, dtype=np.float64)
+    B = weights.shape[0]
+    N, n = pre.D.shape[0], pre.R.shape[0]
+    thr_k = np.array([c.threshold for c in classes], dtype=np.float64)
+    u_hat = np.zeros((N, B))
+    for p in range(B):
+        m = np.ones(N) if masks is None else np.asarray(masks[p], dtype=np.float64)
+        Nkp = np.bincount(pc, weights=m, minlength=len(classes))
+        with np.errstate(divide="ignore", invalid="ignore"):
+            per_class = np.where(Nkp > 0, weights[p, :-1] * thr_k / Nkp, 0.0)
+        u_hat[:, p] = per_class[pc] * m / pre.D
+    b_hat = pre.R[:, None] * weights[None, :, -1]
+    return u_hat, b_hat
+
+
+def admm_run(pre: Preconditioned, u_hat, b_hat, rho, iters: int, tol: Optional[float] = None,
+             eps_abs: float = 1e-6, check_every: int = 10, state0=None, history: bool = False):
+    """Run `iters` iterations (tol=None) or until every plan meets the stopping rule / iters."""
+    A = pre.A_hat
+    n, N = A.shape
+    rho = np.asarray(rho, dtype=np.float64)
+    B = rho.shape[0]
+    if state0 is None:
+        z1 = np.zeros((N, B)); y1 = np.zeros((N, B)); z2 = np.zeros((n, B)); y2 = np.zeros((n, B))
+    else:
+        z1, y1, z2, y2 = (np.array(a, dtype=np.float64, copy=True) for a in state0)
+    c_over_rho = pre.c_hat[:, None] / rho[None, :]
+    active = np.ones(B, dtype=bool)
+    it_done = np.zeros(B, dtype=np.int64)
+    converged = np.zeros(B, dtype=bool)
+    res = np.zeros((B, 2))
+    hist = [] if history else None
+    dim = np.sqrt(float(N + n))
+    for k in range(1, iters + 1):
+        r1 = z1 - y1 - c_over_rho
+        r2 = z2 - y2
+        v = scipy.linalg.cho_solve(pre.chol, A @ r1 - r2)                  # (6)
+        x1 = r1 - A.T @ v                                                  # (7)
+        x2 = v + r2
+        z1n = np.clip(x1 + y1, 0.0, u_hat)                                 # (4b)
+        z2n = np.minimum(x2 + y2, b_hat)
+        y1n = y1 + x1 - z1n                                                # (4c)
+        y2n = y2 + x2 - z2n
+        rp = np.sqrt(np.sum((x1 - z1n) ** 2, axis=0) + np.sum((x2 - z2n) ** 2, axis=0))
+        rd = np.sqrt(np.sum((z1n - z1) ** 2, axis=0) + np.sum((z2n - z2) ** 2, axis=0))
+        nx = np.sqrt(np.sum(x1 ** 2, axis=0) + np.sum(x2 ** 2, axis=0))
+        nz = np.sqrt(np.sum(z1n ** 2, axis=0) + np.sum(z2n ** 2, axis=0))
+        ny = np.sqrt(np.sum(y1n ** 2, axis=0) + np.sum(y2n ** 2, axis=0))
+        a = active
+        z1[:, a] = z1n[:, a]; y1[:, a] = y1n[:, a]; z2[:, a] = z2n[:, a]; y2[:, a] = y2n[:, a]
+        it_done[a] = k
+        res[a, 0] = rp[a]; res[a, 1] = rd[a]
+        if hist is not None:
+            hist.append(np.stack([rp, rd, nx, nz, ny], axis=1))
+        if tol is not None and k % check_every == 0:
+            ok = (rp <= eps_abs * dim + tol * np.maximum(nx, nz)) & (rd <= eps_abs * dim + tol * ny)
+            newly = active & ok
+            converged |= newly
+            active = active & ~ok
+            if not active.any():
+                break
+    out = dict(z1=z1, y1=y1, z2=z2, y2=y2, iters=it_done, converged=converged, res=res)
+    if hist is not None:
+        out["history"] = np.stack(hist, axis=0)        # [iters, B, 5]
+    return out
+
+
+def recover(pre: Preconditioned, state, rho):
+    """t [B, n] = rho * R o y2 (:80) and lambda [B, N] = D o z1 (the dual-LP variables x of Eq. 1)."""
+    rho = np.asarray(rho, dtype=np.float64)
+    t = (state["y2"] * pre.R[:, None] * rho[None, :]).T
+    lam = (state["z1"] * pre.D[:, None]).T
+    return t, lam
+
+
+def solve_workload(w, rho, iters, tol=None, check_every=10, eps_abs=1e-6, pre=None, history=False):
+    """Convenience: precondition + bounds + run + recover + primal objective per plan."""
+    from .lp_model import primal_objective
+    if pre is None:
+        pre = precondition(w.phi, w.point_class, w.classes)
+    masks = None if w.row_mask is None else w.mask_bool()
+    u_hat, b_hat = plan_bounds(pre, w.point_class, w.classes, w.weights, masks)
+    st = admm_run(pre, u_hat, b_hat, rho, iters, tol=tol, eps_abs=eps_abs, check_every=check_every,
+                  history=history)
+    t, lam = recover(pre, st, rho)
+    obj = np.array([primal_objective(w.phi, w.point_class, w.classes, w.weights[p], t[p],
+                                     None if masks is None else masks[p]) for p in range(w.B)])
+    st.update(t=t, lam=lam, obj=obj, pre=pre, u_hat=u_hat, b_hat=b_hat)
+    return st

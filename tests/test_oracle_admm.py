@@ -1,0 +1,189 @@
+"""Pins for O-ADMM (oracle/admm.py).  The paper prints no iterate, so the iteration is pinned by
+what the mathematics fixes: the x-update solved two other ways (Eq. 5 sign-corrected as one KKT
+system; the N x N normal equations of Eq. 4a), invariants, the fixed point at the simplex KKT
+point, metamorphic relations and convergence to the exact LP optimum.  CPU only."""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import admm, lp_model, simplex
+from workloads import default_rho, make_workload
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "c0_simplex_opt.txt")
+
+
+@pytest.fixture(scope="module")
+def small():
+    w = make_workload(0, n_target=180, n_lowdose=320, n_iso=3)       # N=500, n=72, B=9
+    pre = admm.precondition(w.phi, w.point_class, w.classes)
+    u_hat, b_hat = admm.plan_bounds(pre, w.point_class, w.classes, w.weights)
+    rho = default_rho(w.beta)
+    return w, pre, u_hat, b_hat, rho
+
+
+def _x_of_step(before, after):
+    """x^{k+1} from consecutive states via (4c): x = y+ - y + z+."""
+    return (after["y1"] - before["y1"] + after["z1"], after["y2"] - before["y2"] + after["z2"])
+
+
+def test_schur_complement_structure(small):
+    """after row normalisation diag(S) = 2 and off-diagonals lie in [-1, 1]."""
+    _, pre, *_ = small
+    assert np.allclose(np.diag(pre.S), 2.0, atol=1e-12)
+    off = pre.S - np.diag(np.diag(pre.S))
+    assert np.max(np.abs(off)) <= 1.0 + 1e-12
+    assert np.allclose(np.sum(pre.A_hat ** 2, axis=1), 1.0, atol=1e-12)
+
+
+def test_x_update_is_the_constrained_least_squares(small):
+    """(6)+(7) must equal (a) the sign-corrected Eq. (5) solved as one dense system and (b) the
+    minimiser of (4a) from its N x N normal equations (the S' = A^T A + I route of :104)."""
+    w, pre, u_hat, b_hat, rho = small
+    s0 = admm.admm_run(pre, u_hat, b_hat, rho, 7)
+    s1 = admm.admm_run(pre, u_hat, b_hat, rho, 1, state0=(s0["z1"], s0["y1"], s0["z2"], s0["y2"]))
+    x1, x2 = _x_of_step(s0, s1)
+    A = pre.A_hat
+    n, N = A.shape
+    for p in (1, 4, 8):
+        r1 = s0["z1"][:, p] - s0["y1"][:, p] - pre.c_hat / rho[p]
+        r2 = s0["z2"][:, p] - s0["y2"][:, p]
+        K = np.block([[np.eye(N), A.T], [A, -np.eye(n)]])          # Eq. (5) with the (2,2) block -I (R4)
+        sol = np.linalg.solve(K, np.concatenate([r1, r2]))
+        assert np.allclose(sol[:N], x1[:, p], atol=1e-10)
+        assert np.allclose(sol[N:] + r2, x2[:, p], atol=1e-10)    # x2 = v + z2 - y2
+        x1_ne = np.linalg.solve(np.eye(N) + A.T @ A, r1 + A.T @ r2)
+        assert np.allclose(x1_ne, x1[:, p], atol=1e-10)
+        # the PRINTED Eq. (5) (+I) disagrees by O(1): documents the typo reading R4
+        bad = np.linalg.solve(np.block([[np.eye(N), A.T], [A, np.eye(n)]]), np.concatenate([r1, r2]))
+        assert np.max(np.abs(bad[:N] - x1[:, p])) > 1e-3 * np.max(np.abs(x1[:, p]))
+
+
+def test_invariants_every_iteration(small):
+    w, pre, u_hat, b_hat, rho = small
+    st = admm.admm_run(pre, u_hat, b_hat, rho, 0)
+    state = (st["z1"], st["y1"], st["z2"], st["y2"])
+    prev = st
+    for k in range(12):
+        cur = admm.admm_run(pre, u_hat, b_hat, rho, 1, state0=state)
+        x1, x2 = _x_of_step(prev, cur)
+        assert np.allclose(pre.A_hat @ x1, x2, atol=1e-9)                       # (x1,x2) in the set A
+        z1, y1, z2, y2 = cur["z1"], cur["y1"], cur["z2"], cur["y2"]
+        assert np.all(z1 >= 0) and np.all(z1 <= u_hat + 1e-15) and np.all(z2 <= b_hat + 1e-15)
+        assert np.all(y2 >= -1e-15)                                             # multiplier of z2 <= b
+        assert np.all(z1[y1 > 1e-12] == u_hat[y1 > 1e-12])                      # complementarity by construction
+        assert np.all(z1[y1 < -1e-12] == 0.0)
+        assert np.all(z2[y2 > 1e-12] == b_hat[y2 > 1e-12])
+        state = (z1, y1, z2, y2); prev = cur
+
+
+def test_single_state_form_equals_three_variable_form(small):
+    """s = x+ + y  =>  z = Pi(s), y+ = s - z (derived from 4b/4c); the CUDA path stores only s."""
+    w, pre, u_hat, b_hat, rho = small
+    A = pre.A_hat
+    n, N = A.shape
+    B = len(rho)
+    Sinv = np.linalg.inv(pre.S)
+    s1 = np.zeros((N, B)); s2 = np.zeros((n, B))
+    cr = pre.c_hat[:, None] / rho[None, :]
+    for _ in range(40):
+        z1 = np.clip(s1, 0, u_hat); z2 = np.minimum(s2, b_hat)
+        v = Sinv @ (A @ (2 * z1 - s1 - cr) - (2 * z2 - s2))
+        s1 = z1 - cr - A.T @ v
+        s2 = z2 + v
+    ref = admm.admm_run(pre, u_hat, b_hat, rho, 40)
+    assert np.allclose(np.clip(s1, 0, u_hat), ref["z1"], atol=1e-10)
+    assert np.allclose(s1 - np.clip(s1, 0, u_hat), ref["y1"], atol=1e-10)
+    assert np.allclose(np.minimum(s2, b_hat), ref["z2"], atol=1e-9)
+    assert np.allclose(s2 - np.minimum(s2, b_hat), ref["y2"], atol=1e-9)
+
+
+def test_fixed_point_at_simplex_kkt_point(small):
+    """Start at the exact LP solution: z1 = x*/D, y2 = t*/(rho R), y1 = -(c_hat + A_hat^T t_hat)/rho,
+    z2 = A_hat z1.  One iteration must leave it unchanged (z1 -> x*, rho*y2 -> t*)."""
+    w, pre, u_hat, b_hat, rho = small
+    for p in (1, 4, 5, 7):
+        sx = simplex.solve_plan(w.phi, w.point_class, w.classes, w.weights[p])
+        z1 = sx["x"] / pre.D
+        y2 = sx["t"] / (rho[p] * pre.R)
+        y1 = -(pre.c_hat + pre.A_hat.T @ (rho[p] * y2)) / rho[p]
+        z2 = pre.A_hat @ z1
+        st0 = tuple(a[:, None] for a in (z1, y1, z2, y2))
+        out = admm.admm_run(pre, u_hat[:, [p]], b_hat[:, [p]], rho[[p]], 1, state0=st0)
+        scale = max(1.0, np.max(np.abs(y1)))
+        for name, ref in zip(("z1", "y1", "z2", "y2"), st0):
+            assert np.max(np.abs(out[name] - ref)) < 1e-8 * scale, (p, name)
+
+
+def test_objective_scaling_metamorphic(small):
+    """Weights * kappa with rho / kappa: iterates scale by kappa, times t are unchanged."""
+    w, pre, u_hat, b_hat, rho = small
+    kappa = 3.7
+    a = admm.admm_run(pre, u_hat, b_hat, rho, 25)
+    u2, b2 = admm.plan_bounds(pre, w.point_class, w.classes, w.weights * kappa)
+    b = admm.admm_run(pre, u2, b2, rho / kappa, 25)
+    for k in ("z1", "y1", "z2", "y2"):
+        assert np.allclose(b[k], kappa * a[k], rtol=1e-9, atol=1e-12)
+    ta, _ = admm.recover(pre, a, rho); tb, _ = admm.recover(pre, b, rho / kappa)
+    assert np.allclose(ta, tb, rtol=1e-9, atol=1e-14)
+
+
+def test_point_permutation_and_batch_independence(small):
+    w, pre, u_hat, b_hat, rho = small
+    ref = admm.admm_run(pre, u_hat, b_hat, rho, 20)
+    perm = np.random.default_rng(5).permutation(w.N)
+    pre2 = admm.precondition(w.phi[perm], w.point_class[perm], w.classes)
+    u2, b2 = admm.plan_bounds(pre2, w.point_class[perm], w.classes, w.weights)
+    out = admm.admm_run(pre2, u2, b2, rho, 20)
+    assert np.allclose(out["z1"], ref["z1"][perm], atol=1e-10)
+    assert np.allclose(out["y2"], ref["y2"], atol=1e-9)
+    one = admm.admm_run(pre, u_hat[:, [6]], b_hat[:, [6]], rho[[6]], 20)       # plan alone == plan in batch (:96)
+    assert np.allclose(one["z1"][:, 0], ref["z1"][:, 6], atol=1e-12)
+    assert np.allclose(one["y2"][:, 0], ref["y2"][:, 6], atol=1e-12)
+
+
+def test_row_mask_equals_deleting_rows():
+    """zeroing u for rows outside a plan's low-dose set == solving without those rows
+    (same objective; the shared A keeps the rows, so iterates differ but the limit does not)."""
+    w = make_workload(0, n_target=150, n_lowdose=250, n_iso=2)
+    mask = np.ones(w.N, dtype=bool); mask[150::3] = False
+    p = 4
+    full = simplex.solve_plan(w.phi, w.point_class, w.classes, w.weights[p], mask)["opt"]
+    pre = admm.precondition(w.phi, w.point_class, w.classes)
+    u_hat, b_hat = admm.plan_bounds(pre, w.point_class, w.classes, w.weights[[p]], mask[None, :])
+    assert np.all(u_hat[~mask, 0] == 0.0)
+    rho = default_rho(w.beta[[p]])
+    st = admm.admm_run(pre, u_hat, b_hat, rho, 4000, tol=1e-5)
+    t, _ = admm.recover(pre, st, rho)
+    P = lp_model.primal_objective(w.phi, w.point_class, w.classes, w.weights[p], t[0], mask)
+    assert abs(P - full) / max(abs(full), 0.1) < 1e-3
+
+
+def test_converges_to_simplex_optimum_config0():
+    """PAPER.md:80 + north_star: converged objectives within 1e-3 relative of the simplex optimum
+    (error = |P - OPT| / max(|OPT|, 0.1), reading R15).  beta > 0 plans of config 0."""
+    g = np.loadtxt(GOLDEN)
+    plans = [1, 2, 4, 5, 7, 8, 0]
+    w = make_workload(0, plans=plans)
+    rho = default_rho(w.beta)
+    st = admm.solve_workload(w, rho, 3000, tol=1e-4)
+    assert st["converged"].all()
+    assert np.all(st["iters"] % 10 == 0)
+    err = np.abs(st["obj"] - g[plans, 3]) / np.maximum(np.abs(g[plans, 3]), 0.1)
+    assert np.all(err < 1e-3), err
+    # and the weak-duality bracket closes: Dual(lambda) <= OPT <= P(t)
+    masks = None
+    for i, p in enumerate(plans[:3]):
+        lo = lp_model.dual_bound(w.phi, w.point_class, w.classes, w.weights[i], st["lam"][i])
+        assert lo <= g[p, 3] + 1e-9 <= st["obj"][i] + 2e-9
+        assert (st["obj"][i] - lo) / max(abs(st["obj"][i]), 0.1) < 2e-3
+
+
+def test_stopping_rule_freezes_converged_plans(small):
+    w, pre, u_hat, b_hat, rho = small
+    a = admm.admm_run(pre, u_hat, b_hat, rho, 400, tol=1e-3, check_every=10)
+    assert a["converged"].any() and not np.all(a["iters"] == a["iters"][0])
+    p = int(np.argmin(a["iters"]))
+    k = int(a["iters"][p])
+    b = admm.admm_run(pre, u_hat, b_hat, rho, k)                                # frozen state == state after k its
+    assert np.array_equal(a["z1"][:, p], b["z1"][:, p]) and np.array_equal(a["y2"][:, p], b["y2"][:, p])

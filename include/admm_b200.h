@@ -1,0 +1,174 @@
+/*
+ * admm_b200.h -- C ABI of the B200-native batched ADMM solver for the Lightning-style
+ * radiosurgery LP (arXiv 2509.08602).  One GPU, CUDA sm_100a.  No torch types, plain
+ * pointers and sizes only.  Citations are PAPER.md line numbers (section / equation).
+ *
+ * The problem (App. A :308-344).  For plan p with class
+ * weights w_k (dose units), beam-on-time weight w_BOT and an optional per-plan row mask:
+ *
+ *   P_p(t) = sum_k (w_k / N_{k,p}) sum_{i in class k, active in p} max(0, s_k (thr_k - Phi_i t))
+ *            + w_BOT sum_j t_j ,   t >= 0
+ *
+ * solved through its dual  min c^T x, A x <= b, 0 <= x <= u  (Eq. 1, :47-49) by the ADMM
+ * iteration Eq. (4b), (4c), (6), (7) (:70-94), all B plans at once (:96-98), one rho per
+ * plan (:222), S = A A^T + I inverted once per handle and shared by every plan (:91).
+ *
+ * Threading: one handle is not thread-safe; distinct handles are independent.
+ * Errors: every entry point returns a status; nothing throws or aborts across the ABI; on
+ * error the outputs are untouched and admm_last_error() describes the failure.
+ * There is no CPU fallback: without a CUDA sm_100 device every call fails with ADMM_ECUDA.
+ */
+#ifndef ADMM_B200_H
+#define ADMM_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct admm_handle admm_handle;   /* opaque; one per (Phi, point classes) */
+
+typedef enum {
+    ADMM_OK = 0,
+    ADMM_EINVAL = 1,    /* bad argument (null pointer, non-finite weight, B < 1, ...) */
+    ADMM_ENOMEM = 2,    /* device or host allocation failed */
+    ADMM_ECUDA = 3,     /* CUDA / cuBLAS / cuSOLVER error, or no sm_100 device */
+    ADMM_ENOTSPD = 4,   /* Cholesky of S failed (cannot happen for finite Phi: lambda_min(S) >= 1) */
+    ADMM_ESTATE = 5     /* call order violated (e.g. admm_get_state before any solve) */
+} admm_status;
+
+/* One dose-point class (Eq. 11-15 :314-326).
+ * sense = +1: "dose >= threshold", under-dose is penalised (target surface / interior);
+ * sense = -1: "dose <= threshold", over-dose is penalised (ring, low-dose volumes).
+ * hard  = 1 : u = infinity (OAR-style hard constraint, Eq. 15).  Accepted by the ABI, rejected
+ *             with ADMM_EINVAL by this build (not on the hot path). */
+typedef struct {
+    int32_t sense;
+    float   threshold;
+    int32_t hard;
+} admm_class;
+
+/* How Phi is stored in HBM and consumed by the tensor cores (BASELINE.json config 4). */
+enum {
+    ADMM_STORAGE_FP32_3XTF32 = 0, /* fp32 storage, hi/lo split on chip, 3 tf32 MMAs: the fp32 path (1e-4 parity) */
+    ADMM_STORAGE_FP32_TF32   = 1, /* Phi rounded once to tf32 (kept in an fp32 container), 2 tf32 MMAs */
+    ADMM_STORAGE_BF16        = 2, /* Phi rounded once to bf16, bf16 MMAs (1e-2 parity)  [not built yet] */
+    ADMM_STORAGE_CSR         = 3  /* thresholded CSR                                     [not built yet] */
+};
+
+/* Which kernels run the two Phi contractions. */
+enum {
+    ADMM_PATH_TCGEN05 = 0,        /* tcgen05/TMEM/TMA kernels (the product path) */
+    ADMM_PATH_SIMT    = 1         /* plain fp32 FFMA kernels: a slow on-device cross-check, same ABI */
+};
+
+typedef struct {
+    int32_t storage;           /* ADMM_STORAGE_*                                                    */
+    int32_t kernel_path;       /* ADMM_PATH_*                                                       */
+    int32_t device;            /* CUDA device ordinal                                               */
+    void*   stream;            /* cudaStream_t all work is enqueued on; NULL = the legacy default stream */
+    int32_t check_every;       /* stopping rule tested every this many iterations; 0 => 10          */
+    float   eps_abs;           /* absolute part of the stopping rule; 0 => 1e-6 (reading R7) */
+    int32_t compaction;        /* 1: converged plans are swapped out of the active batch; 0: masked only */
+    float   csr_rel_threshold; /* ADMM_STORAGE_CSR only                                             */
+    int32_t profile_kernels;   /* 1: CUDA events around every hot-path kernel (admm_get_kernel_times) */
+    int32_t reserved[7];       /* must be 0 */
+} admm_options;
+
+/* Fills *opt with the defaults (3xTF32, tcgen05 path, device 0, default stream, check 10, 1e-6, compaction on). */
+void admm_default_options(admm_options* opt);
+
+/*
+ * Setup, steps S0-S2 of DESIGN.md ("compute its inverse just once and cache it",
+ * :183/:213 row/column scaling).  Copies Phi into library-owned HBM (plus its transpose), builds
+ * the preconditioner D_i = 1/N_class(i), R_j = 1/||row j of A D||_2, forms S = I + A^ A^^T in fp64,
+ * Cholesky-factorises and inverts it in fp64.  Shared by every later admm_solve_batch.
+ *
+ *   phi            [N][ld] fp32 row-major, Phi[i][j] = dose rate at point i per unit of time variable j
+ *                  (>= 0, finite).  Host pointer if phi_on_device == 0, else device pointer.
+ *                  The caller keeps ownership; the library holds no reference after return.
+ *   N, n, ld       points, time variables, row stride in elements (ld >= n)
+ *   point_class    [N] HOST uint8, class id of each point, < n_classes
+ *   classes        [n_classes] HOST, 1 <= n_classes <= 8
+ *   opt            NULL => defaults
+ * On success *out is a new handle (free with admm_destroy).
+ */
+admm_status admm_setup(admm_handle** out, const float* phi, int32_t phi_on_device,
+                       int64_t N, int64_t n, int64_t ld,
+                       const uint8_t* point_class, const admm_class* classes, int32_t n_classes,
+                       const admm_options* opt);
+
+/*
+ * Solve B plans at once: steps H1-H6 of DESIGN.md = Eq. (6), (7), (4b), (4c) per iteration
+ * (PAPER.md:73-94), stacked per :96, from the all-zero iterate.
+ *
+ *   weights     [B][n_classes+1] HOST fp32: w_class 0.., then w_BOT (config LP: 1, alpha, beta); >= 0, finite
+ *   rho         [B] HOST fp32 step sizes (> 0), or NULL => rho0*sqrt(w0/max(w_BOT,w0)), rho0=1e-3, w0=0.05
+ *               (the shape of Eq. 9, :219)
+ *   row_mask    [B][ceil(N/32)] uint32 bit-packed (bit i%32 of word i/32 set => row i active in plan p;
+ *               inactive rows get u = 0, :144), HOST or DEVICE pointer, or NULL => all rows active
+ *   tol         relative tolerance of the stopping rule (R7); ignored if fixed_iters > 0
+ *   max_iter    iteration cap (>= 1) when fixed_iters == 0
+ *   fixed_iters > 0 => run exactly this many iterations for every plan, no masking, no compaction
+ * Outputs (HOST or DEVICE pointers, detected; any may be NULL to skip):
+ *   t_out       [B][n] fp32 beam-on times t_p = rho_p * R o y2_p (:80)
+ *   obj_out     [B] fp64 primal objective P_p(t_p)
+ *   res_out     [B][2] fp32 primal / dual residual norms ||x - z||, ||z+ - z|| at the plan's last tested iterate
+ *   iters_out   [B] int32 iterations done (a multiple of check_every if the plan converged)
+ * Synchronises opt->stream before returning.
+ */
+admm_status admm_solve_batch(admm_handle* h, int32_t B,
+                             const float* weights, const float* rho, const uint32_t* row_mask,
+                             float tol, int32_t max_iter, int32_t fixed_iters,
+                             float* t_out, double* obj_out, float* res_out, int32_t* iters_out);
+
+/*
+ * Parity hook: the iterate of plan `plan` of the LAST admm_solve_batch in the paper's three-variable
+ * form, recovered from the stored single state s = x + y (z = Pi(s), y = s - z):
+ *   z1, y1 [N] fp32 ;  z2, y2 [n] fp64   (HOST or DEVICE pointers; any may be NULL)
+ */
+admm_status admm_get_state(admm_handle* h, int32_t plan, float* z1, float* y1, double* z2, double* y2);
+
+/*
+ * Test hook: ONE raw dose-rate contraction through the kernels of the selected path, no ADMM arithmetic.
+ *   which = 0:  out[B][n] = small[B][N] . Phi      (the product of Eq. 6, before row scaling)
+ *   which = 1:  out[B][N] = small[B][n] . Phi^T    (the product of Eq. 7)
+ * small: HOST fp32 [B][K]; out: HOST fp64; 1 <= B <= 256.  Invalidates the state of the last solve.
+ */
+admm_status admm_contract_probe(admm_handle* h, int32_t which, int32_t B, const float* small, double* out);
+
+/* Copies the preconditioner (fp64, HOST pointers, any may be NULL): D [N], R [n], Sinv [n][n]. */
+admm_status admm_get_preconditioner(admm_handle* h, double* D, double* R, double* Sinv);
+
+/*
+ * Wall/device times of the last calls, milliseconds:
+ *   ms[0] upload+transpose  ms[1] S = I + A^A^^T (syrk)  ms[2] Cholesky + inverse  ms[3] setup total
+ *   ms[4] last solve: iterations (device)   ms[5] last solve: finalise (device)   ms[6] last solve total (host wall)
+ *   ms[7] reserved
+ *   plan_iters = sum over plans of iterations done in the last solve.
+ */
+admm_status admm_get_timing(admm_handle* h, double ms[8], int64_t* plan_iters);
+
+/*
+ * Per-kernel device time of the last solve when opt.profile_kernels = 1 (CUDA events on the
+ * launching stream around every launch): for k in {0: K1 Phi^T.G, 1: K2 S^-1 apply, 2: K3 Phi.V + epilogue,
+ * 3: convergence/compaction}: total_ms[k], launches[k].
+ */
+admm_status admm_get_kernel_times(admm_handle* h, double total_ms[4], int64_t launches[4]);
+
+/* Number of kernels the library launched in the last solve (all of them its own). */
+int64_t admm_last_launch_count(const admm_handle* h);
+
+/* Message of the last error on this handle (or of the last failed admm_setup if h == NULL). Never NULL. */
+const char* admm_last_error(const admm_handle* h);
+
+void admm_destroy(admm_handle* h);
+
+/* "paper_2509_08602_b200 <version> sm_100a" */
+const char* admm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ADMM_B200_H */

@@ -1,0 +1,156 @@
+// Internal declarations shared by the translation units of libadmm_b200.so.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/admm_b200.h"
+
+constexpr int kMaxClasses = 8;
+constexpr int kTileM = 128;        // rows of the big (Phi-side) operand per UMMA tile
+constexpr int kBlockK = 32;        // fp32 elements per k-block = one 128-byte swizzle row
+constexpr int kBoxRows = 32;       // rows per TMA box of the big operand (partial tiles load fewer boxes)
+constexpr int kMaxBpad = 512;      // slots in the per-plan tables / partial-sum arrays (B <= 512)
+constexpr int kMaxMmaN = 256;      // plans per contraction pass (UMMA N limit); larger batches run in chunks
+constexpr int kNumResid = 5;       // ||x-z+||^2, ||z+-z||^2, ||x||^2, ||z+||^2, ||y+||^2
+
+// One unit of work of a contraction kernel: a 128-row tile of the big operand times a k-range.
+struct TcUnit {
+    int32_t row0;      // first row of the tile in the big operand
+    int32_t rows;      // valid rows (1..128)
+    int32_t kb0;       // first k-block (of 32 elements)
+    int32_t kb_count;  // number of k-blocks (>= 1)
+    int32_t slot;      // K1: partial-sum slot this unit writes
+    int32_t pad;
+};
+
+// Epilogue selector of the contraction kernels
+enum { EPI_K1_PARTIAL = 0, EPI_K3_STATE = 1, EPI_OBJECTIVE = 2, EPI_RAW = 3 };
+
+// Everything the epilogues need.  Plan-major ("slot-major") layouts: a plan's vector is contiguous.
+struct EpiParams {
+    // common
+    int32_t slot0;              // first slot of this contraction pass (chunk of <= 256 plans)
+    int32_t n_slots_active;     // live slots of this pass: slot0 .. slot0 + n_slots_active - 1
+    int32_t n_mma;              // UMMA N (multiple of 16, >= n_slots_active)
+    int64_t N, n;               // points, time variables
+    int64_t ldN, ldn;           // row strides of [slot][N] and [slot][n] arrays (elements)
+    // K1: partial[slot][plan][128] fp32
+    float* partial;
+    // K3 / objective
+    const uint8_t* point_class;     // [N]
+    const uint32_t* mask;           // [B][mask_words] or nullptr
+    const int32_t* slot_plan;       // [Bpad] plan index of each slot (mask row)
+    int64_t mask_words;
+    const float* utab;              // [kMaxClasses][kMaxBpad] u_hat per (class, slot)
+    const float* crtab;             // [kMaxClasses][kMaxBpad] c_hat / rho per (class, slot)
+    float a_cls[kMaxClasses];       // sigma_k * D_k
+    float sense[kMaxClasses];
+    float thr[kMaxClasses];
+    float* s1;                      // [Bpad][ldN] single state s = x + y of block 1
+    float* g_hi;                    // [Bpad][ldN] operand of K1: tf32 head of a (2 z1 - s1 - c/rho)
+    float* g_lo;                    // [Bpad][ldN] tail
+    float* resid_partial;           // [grid][kMaxBpad][kNumResid] per-CTA residual sums (nullptr: not this iteration)
+    double* hinge_partial;          // objective: [grid][kMaxBpad][kMaxClasses]
+    float* qraw;                    // EPI_RAW (test hook): raw accumulators [slot][ldN]
+};
+
+struct TcLaunch {
+    CUtensorMap map_big;     // big operand [rows][K], box {32, 32}
+    CUtensorMap map_small_hi;// small operand [Bpad][K], box {32, n_mma}
+    CUtensorMap map_small_lo;
+    const TcUnit* units;     // device
+    const int32_t* cta_unit_begin;  // device [grid + 1]
+    int32_t grid;
+    int32_t mma_passes;      // 3: 3xTF32 with on-chip split of the big operand; 2: big operand already on the tf32 grid
+    int32_t epi;
+    int32_t chunk_kb;        // > 0: drain the TMEM accumulator every chunk_kb k-blocks (fp32 path, n_mma <= 128); 0: never
+    EpiParams ep;
+};
+
+struct KernelTimes {
+    double total_ms[4] = {0, 0, 0, 0};
+    int64_t launches[4] = {0, 0, 0, 0};
+};
+
+struct admm_handle {
+    admm_options opt{};
+    cudaStream_t stream = nullptr;
+    int sm_count = 148;
+    int64_t N = 0, n = 0, ldN = 0, ldn = 0;
+    int n_classes = 0;
+    admm_class classes[kMaxClasses]{};
+    int64_t class_count[kMaxClasses]{};
+    std::vector<uint8_t> h_point_class;
+
+    // device, owned
+    float* d_phi = nullptr;        // [N][ldn]
+    float* d_phiT = nullptr;       // [n][ldN]
+    uint8_t* d_point_class = nullptr;
+    double* d_R = nullptr;         // [n]
+    double* d_Sinv = nullptr;      // [n][n]
+    std::vector<double> h_R;
+
+    // per-solve state (reallocated when B grows)
+    int32_t B = 0, Bpad = 0;
+    float *d_s1 = nullptr, *d_ghi = nullptr, *d_glo = nullptr;        // [Bpad][ldN]
+    double* d_s2 = nullptr;                                           // [Bpad][ldn]
+    double* d_rhs = nullptr;                                          // [Bpad][ldn]
+    float *d_vhi = nullptr, *d_vlo = nullptr;                         // [Bpad][ldn]
+    float* d_partial = nullptr; int64_t partial_slots = 0;            // [slots][Bpad][128]
+    float* d_resid1 = nullptr;                                        // [grid][kMaxBpad][5]
+    double* d_resid2 = nullptr;                                       // [blocks][kMaxBpad][5]
+    double* d_hinge = nullptr;                                        // [grid][kMaxBpad][kMaxClasses]
+    uint32_t* d_mask = nullptr; int64_t mask_words = 0; bool has_mask = false;
+    int32_t* d_slot_plan = nullptr;
+    float *d_utab = nullptr, *d_crtab = nullptr;
+    double *d_beta = nullptr, *d_rho = nullptr;                       // per slot
+    int32_t* d_active_counts = nullptr;                               // [B][kMaxClasses]
+    int32_t* d_conv_flags = nullptr;                                  // [Bpad] + counter
+    float* d_res_slot = nullptr;                                      // [Bpad][2]
+    float* d_rowtmp = nullptr; double* d_rowtmp2 = nullptr;
+    TcUnit* d_units_k1 = nullptr; int32_t* d_cta_begin_k1 = nullptr; int grid_k1 = 0; int slots_k1 = 0;
+    int32_t* d_mtile_slot_begin = nullptr;                            // [m_tiles + 1]
+    TcUnit* d_units_k3 = nullptr; int32_t* d_cta_begin_k3 = nullptr; int grid_k3 = 0;
+    std::vector<int32_t> slot_plan, plan_slot, iters;
+    std::vector<double> h_beta, h_rho;
+    std::vector<float> h_weights;
+    bool solved = false;
+
+    double ms[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int64_t plan_iters = 0;
+    int64_t launch_count = 0;
+    KernelTimes ktimes;
+    std::string err;
+};
+
+// ---- gemm_tc.cu
+admm_status tc_init(admm_handle* h);                       // resolves cuTensorMapEncodeTiled, sets smem attribute
+admm_status tc_make_map(admm_handle* h, CUtensorMap* out, const void* base, int64_t rows, int64_t cols,
+                        int64_t ld_elems, int box_rows);
+admm_status tc_launch(admm_handle* h, const TcLaunch& L);
+
+// ---- kernels.cu  (everything that is not a tcgen05 contraction)
+void launch_transpose(const float* src, int64_t rows, int64_t cols, int64_t ld_src, float* dst, int64_t ld_dst, cudaStream_t s);
+void launch_scale_rows_to_f64(const float* phi, int64_t ld, int64_t row0, int64_t rows, int64_t n,
+                              const uint8_t* cls, const double* a_cls, double* out, cudaStream_t s);
+void launch_round_tf32(float* x, int64_t count, cudaStream_t s);
+void launch_finish_S(double* M, int64_t n, double* R, cudaStream_t s);      // M -> S = I + R M R (in place), R from diag
+void launch_symmetrize(double* A, int64_t n, cudaStream_t s);
+void launch_count_active(const uint32_t* mask, int64_t mask_words, const uint8_t* cls, int64_t N, int B,
+                         int32_t* counts, cudaStream_t s);
+void launch_emit_g(const EpiParams& ep, int Bact, cudaStream_t s);          // G from the current s1 (start / warm start)
+void launch_k2a(admm_handle* h, int slot0, int nact, int n_mma, cudaStream_t s);
+void launch_k2b(admm_handle* h, int Bact, bool resid, cudaStream_t s);
+void launch_simt_k1(admm_handle* h, int slot0, int nact, int n_mma, int splits, cudaStream_t s);
+void launch_simt_k3(admm_handle* h, const EpiParams& ep, int epi, const float* vhi, const float* vlo, float* qbuf, cudaStream_t s);
+void launch_convergence(admm_handle* h, int Bact, int grid1, int grid2, float tol, float eps_abs, cudaStream_t s);
+void launch_make_t(admm_handle* h, int Bact, float* t_hi, float* t_lo, float* t_f32, cudaStream_t s);
+void launch_objective_reduce(admm_handle* h, int B, int grid, const float* t_f32, const double* wnorm, double* obj_slot, cudaStream_t s);
+void launch_gather_rows(const float* src, int64_t ld, const int32_t* plan_slot, int B, int64_t n, float* dst, cudaStream_t s);
+void launch_state_out(admm_handle* h, const EpiParams& ep, int slot, double beta, float* z1, float* y1, double* z2, double* y2, cudaStream_t s);
+int k2b_grid(const admm_handle* h, int Bact);
+void launch_split_tf32(const float* x, int64_t count, float* hi, float* lo, cudaStream_t s);
+void launch_reduce_partial(admm_handle* h, int nact, int n_mma, double* out, cudaStream_t s);

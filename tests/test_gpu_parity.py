@@ -1,0 +1,242 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the fp64 CPU oracle, element by element, on the
+same seeded inputs.  Tolerances (north_star): iterates after a fixed K = 50 iterations within 1e-4 relative
+(fp32 path; metric = DESIGN.md reading R17), converged objectives within 1e-3 relative of the simplex optimum
+(error = |P - OPT| / max(|OPT|, 0.1), reading R15)."""
+import os
+
+import numpy as np
+import pytest
+
+from conftest import have_cuda
+from parity_util import stacked_errors, t_errors
+
+pytestmark = [pytest.mark.gpu, pytest.mark.skipif(not have_cuda(), reason="needs a CUDA device")]
+
+TOL_FP32 = 1e-4
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "c0_simplex_opt.txt")
+
+
+@pytest.fixture(scope="module")
+def b():
+    from paper_2509_08602_b200 import binding
+    return binding
+
+
+def _oracle(w, rho, K, **kw):
+    from oracle import admm
+    return admm.solve_workload(w, rho, K, **kw)
+
+
+def _gpu_states(b, h, B):
+    return [b.admm_get_state(h, p) for p in range(B)]
+
+
+def _parity(b, w, rho, K, ref=None, **setup_kw):
+    ref = ref if ref is not None else _oracle(w, rho, K)
+    h = b.admm_setup(w.phi, w.point_class, w.classes, **setup_kw)
+    out = b.admm_solve_batch(h, w.weights, rho, w.row_mask, fixed_iters=K)
+    ez, ey = stacked_errors(_gpu_states(b, h, w.B), ref)
+    et = t_errors(out["t"], ref["t"])
+    eobj = np.abs(out["obj"] - ref["obj"]) / np.maximum(np.abs(ref["obj"]), 0.1)
+    launches = b.admm_last_launch_count(h)
+    h.close()
+    return ez, ey, et, eobj, out, launches
+
+
+# ------------------------------------------------------------------------------------------ the contraction alone
+@pytest.mark.parametrize("shape", [dict(n_target=700, n_lowdose=1400, n_iso=10),      # N=2100 (16 full tiles + 52 rows), n=240
+                                   dict(n_target=333, n_lowdose=1001, n_iso=7),       # N=1334, n=168: ragged in both dims
+                                   dict(n_target=40, n_lowdose=57, n_iso=1)])         # N=97 < one tile, n=24 < one k-block
+def test_contractions_match_fp64_matmul(b, shape):
+    from workloads import make_workload
+    w = make_workload(0, **shape)
+    rng = np.random.default_rng(1)
+    P = w.phi.astype(np.float64)
+    h = b.admm_setup(w.phi, w.point_class, w.classes)
+    for which, Bp in ((1, 9), (0, 16), (1, 81), (0, 81), (1, 128)):
+        K = w.N if which == 0 else w.n
+        small = rng.standard_normal((Bp, K)).astype(np.float32)
+        got = b.admm_contract_probe(h, which, small)
+        exact = small.astype(np.float64) @ (P if which == 0 else P.T)
+        scale = np.abs(small.astype(np.float64)) @ (P if which == 0 else P.T)    # sum of |terms| per output
+        assert np.max(np.abs(got - exact) / scale) < 1e-6, (which, Bp)
+    h.close()
+
+
+def test_accumulation_is_unbiased(b):
+    """tcgen05.mma accumulates with round-toward-zero; the drained fp32 path must not show that bias
+    (all-positive operands, K = 4800: undrained it is -3e-5 of the sum)."""
+    from workloads import make_workload
+    w = make_workload(0, n_target=300, n_lowdose=500, n_iso=200)
+    small = np.abs(np.random.default_rng(2).standard_normal((16, w.n))).astype(np.float32)
+    h = b.admm_setup(w.phi, w.point_class, w.classes)
+    got = b.admm_contract_probe(h, 1, small)
+    h.close()
+    exact = small.astype(np.float64) @ w.phi.astype(np.float64).T
+    rel = (got - exact) / exact
+    assert abs(np.mean(rel)) < 1e-7 and np.max(np.abs(rel)) < 1e-6
+
+
+# ------------------------------------------------------------------------------------------ fixed-K iterate parity
+def test_fixed_k_parity_config0(b):
+    from workloads import default_rho, make_workload
+    w = make_workload(0)                                         # BASELINE.json configs[0], all 9 plans
+    ez, ey, et, eobj, out, launches = _parity(b, w, default_rho(w.beta), 50)
+    assert launches > 0
+    assert ez.max() < TOL_FP32 and ey.max() < TOL_FP32 and et.max() < TOL_FP32, (ez, ey, et)
+    assert eobj.max() < 1e-4
+    assert np.all(out["iters"] == 50)
+
+
+def test_fixed_k_parity_several_tiles_ragged_tail(b):
+    from workloads import default_rho, make_workload
+    w = make_workload(1, n_target=2000, n_lowdose=4100, n_iso=7)  # N=6100 (ragged), n=168 (ragged), B=81
+    ez, ey, et, eobj, _, _ = _parity(b, w, default_rho(w.beta), 50)
+    assert ez.max() < TOL_FP32 and ey.max() < TOL_FP32 and et.max() < TOL_FP32, (ez.max(), ey.max(), et.max())
+
+
+def test_fixed_k_parity_row_masks_multitarget(b):
+    from workloads import default_rho, make_workload
+    w = make_workload(2, n_target=1500, n_lowdose=3000, n_iso=18, grid=5)   # 9 targets, per-plan low-dose masks, B=25
+    assert w.row_mask is not None
+    ez, ey, et, eobj, _, _ = _parity(b, w, default_rho(w.beta), 50)
+    assert ez.max() < TOL_FP32 and ey.max() < TOL_FP32 and et.max() < TOL_FP32, (ez.max(), ey.max(), et.max())
+
+
+def test_fixed_k_parity_more_than_one_pass_of_plans(b):
+    """B = 144 > 128: the fp32 path runs the contractions in two passes over the plans."""
+    from workloads import default_rho, make_workload
+    w = make_workload(0, n_target=600, n_lowdose=1200, n_iso=4, grid=12)
+    ez, ey, et, _, _, _ = _parity(b, w, default_rho(w.beta), 30)
+    assert ez.max() < TOL_FP32 and ey.max() < TOL_FP32 and et.max() < TOL_FP32
+
+
+def test_simt_cross_check_path(b):
+    from workloads import default_rho, make_workload
+    w = make_workload(0, n_target=500, n_lowdose=900, n_iso=5)
+    ez, ey, et, _, _, _ = _parity(b, w, default_rho(w.beta), 50, kernel_path=b.ADMM_PATH_SIMT)
+    assert ez.max() < TOL_FP32 and ey.max() < TOL_FP32 and et.max() < TOL_FP32
+
+
+def test_tf32_storage_parity_against_same_rounded_phi(b):
+    """ADMM_STORAGE_FP32_TF32 (reading R18): against the oracle fed the SAME tf32-rounded Phi the only difference
+    is arithmetic; against the original Phi it must stay inside the 1e-2 reduced-storage budget."""
+    from workloads import default_rho, make_workload
+    w = make_workload(0, n_target=700, n_lowdose=1400, n_iso=6)
+    rho = default_rho(w.beta)
+    u = w.phi.view(np.uint32).astype(np.uint64)
+    rounded = (((u + 0xFFF + ((u >> 13) & 1)) & 0xFFFFE000).astype(np.uint32)).view(np.float32)
+    import copy
+    wr = copy.copy(w); wr.phi = rounded
+    ref_same = _oracle(wr, rho, 50)
+    ez, ey, et, _, _, _ = _parity(b, w, rho, 50, ref=ref_same, storage=b.ADMM_STORAGE_FP32_TF32)
+    assert ez.max() < 1e-3 and ey.max() < 1e-3 and et.max() < 2e-3, (ez.max(), ey.max(), et.max())
+    ez, ey, et, _, _, _ = _parity(b, w, rho, 50, storage=b.ADMM_STORAGE_FP32_TF32)
+    assert ez.max() < 1e-2 and ey.max() < 1e-2 and et.max() < 1e-2
+
+
+# ------------------------------------------------------------------------------------------ setup
+def test_preconditioner_matches_oracle(b):
+    from oracle import admm
+    from workloads import make_workload
+    w = make_workload(0, n_target=400, n_lowdose=800, n_iso=6)
+    pre = admm.precondition(w.phi, w.point_class, w.classes)
+    h = b.admm_setup(w.phi, w.point_class, w.classes)
+    D, R, Sinv = b.admm_get_preconditioner(h)
+    h.close()
+    assert np.allclose(D, pre.D, rtol=1e-15) and np.allclose(R, pre.R, rtol=1e-12)
+    assert np.max(np.abs(Sinv @ pre.S - np.eye(w.n))) < 1e-10
+    assert np.allclose(Sinv, Sinv.T, atol=0)
+
+
+# ------------------------------------------------------------------------------------------ convergence, masking, compaction
+def test_converged_objectives_match_simplex_config0(b):
+    from workloads import default_rho, make_workload
+    g = np.loadtxt(GOLDEN)
+    w = make_workload(0)
+    rho = default_rho(w.beta)
+    h = b.admm_setup(w.phi, w.point_class, w.classes)
+    out = b.admm_solve_batch(h, w.weights, rho, tol=1e-4, max_iter=3000)
+    h.close()
+    err = np.abs(out["obj"] - g[:, 3]) / np.maximum(np.abs(g[:, 3]), 0.1)
+    conv = out["iters"] < 3000
+    assert conv.sum() >= 7 and np.all(out["iters"][conv] % 10 == 0)
+    assert np.all(err[conv] < 1e-3), err
+    # iteration counts: the decision is taken on fp32 data, the oracle's in fp64 -> same count up to one test interval
+    ref = _oracle(w, rho, 3000, tol=1e-4)
+    both = conv & ref["converged"]
+    assert both.sum() >= 7
+    assert np.all(np.abs(out["iters"][both] - ref["iters"][both]) <= 20), (out["iters"], ref["iters"])
+
+
+def test_compaction_preserves_each_plan(b):
+    """A plan frozen and swapped out at iteration k must equal the same plan run alone for k iterations,
+    and plans that keep iterating must not be disturbed by the swaps (plans are independent columns, :96)."""
+    from workloads import default_rho, make_workload
+    w = make_workload(0, n_target=500, n_lowdose=900, n_iso=5)
+    rho = default_rho(w.beta)
+    h = b.admm_setup(w.phi, w.point_class, w.classes)
+    out = b.admm_solve_batch(h, w.weights, rho, tol=1e-3, max_iter=400)
+    iters = out["iters"].copy()
+    states = _gpu_states(b, h, w.B)
+    assert len(set(iters.tolist())) > 2                      # plans really stopped at different iterations
+    for p in (int(np.argmin(iters)), int(np.argmax(iters)), 4):
+        one = w.subset([p])
+        o1 = b.admm_solve_batch(h, one.weights, rho[[p]], fixed_iters=int(iters[p]))
+        z1, y1, z2, y2 = b.admm_get_state(h, 0)
+        assert np.array_equal(z1, states[p][0]) and np.array_equal(y1, states[p][1])
+        assert np.array_equal(z2, states[p][2]) and np.array_equal(y2, states[p][3])
+        assert np.array_equal(o1["t"][0], out["t"][p])
+    h.close()
+
+
+def test_residuals_match_oracle(b):
+    from workloads import default_rho, make_workload
+    w = make_workload(0, n_target=500, n_lowdose=900, n_iso=5)
+    rho = default_rho(w.beta)
+    ref = _oracle(w, rho, 40)
+    h = b.admm_setup(w.phi, w.point_class, w.classes)
+    out = b.admm_solve_batch(h, w.weights, rho, fixed_iters=40)
+    h.close()
+    big = ref["res"] > 1e-3
+    assert np.allclose(out["res"][big], ref["res"][big], rtol=2e-3)
+
+
+# ------------------------------------------------------------------------------------------ ABI behaviour on the device
+def test_device_buffers_and_errors(b):
+    import torch
+    from workloads import default_rho, make_workload
+    w = make_workload(2, n_target=600, n_lowdose=1200, n_iso=9, grid=3)
+    rho = default_rho(w.beta)
+    dev = torch.device("cuda", 0)
+    phi_d = torch.from_numpy(w.phi).to(dev)
+    mask_d = torch.from_numpy(w.row_mask.view(np.int32)).to(dev)
+    h = b.admm_setup(phi_d, w.point_class, w.classes)
+    with pytest.raises(b.AdmmError) as e:
+        b.admm_get_state(h, 0)
+    assert e.value.status == b.ADMM_ESTATE
+    outs = dict(t=torch.full((w.B, w.n), -7.0, dtype=torch.float32, device=dev),
+                obj=torch.zeros(w.B, dtype=torch.float64, device=dev))
+    with pytest.raises(b.AdmmError) as e:                         # bad weight: outputs untouched
+        bad = w.weights.copy(); bad[0, 0] = -1.0
+        b.admm_solve_batch(h, bad, rho, mask_d, fixed_iters=5, out=outs)
+    assert e.value.status == b.ADMM_EINVAL and float(outs["t"].min()) == -7.0
+    o_dev = b.admm_solve_batch(h, w.weights, rho, mask_d, fixed_iters=20, out=outs)
+    h.close()
+    h2 = b.admm_setup(w.phi, w.point_class, w.classes)
+    o_host = b.admm_solve_batch(h2, w.weights, rho, w.row_mask, fixed_iters=20)
+    h2.close()
+    assert np.array_equal(o_dev["t"].cpu().numpy(), o_host["t"]) and np.array_equal(o_dev["obj"].cpu().numpy(), o_host["obj"])
+
+
+def test_single_plan_and_degenerate_weights(b):
+    """B = 1; alpha = beta = 0 (optimum 0, every iterate of z stays 0); beta large (t* = 0, OPT = 1)."""
+    from workloads import make_workload
+    w = make_workload(0, n_target=300, n_lowdose=500, n_iso=4)
+    h = b.admm_setup(w.phi, w.point_class, w.classes)
+    out = b.admm_solve_batch(h, np.array([[1.0, 0.0, 0.0]]), np.array([1e-3]), tol=1e-4, max_iter=500)
+    assert out["obj"][0] < 1e-6 and out["iters"][0] <= 100
+    bound = w.phi[w.point_class == 0].astype(np.float64).mean(axis=0).max()
+    out = b.admm_solve_batch(h, np.array([[1.0, 0.5, 1.5 * bound]]), None, tol=1e-4, max_iter=3000)
+    assert abs(out["obj"][0] - 1.0) < 1e-3 and np.max(np.abs(out["t"])) < 1e-3
+    h.close()

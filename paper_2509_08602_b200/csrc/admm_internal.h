@@ -59,6 +59,7 @@ struct EpiParams {
 
 struct TcLaunch {
     CUtensorMap map_big;     // big operand [rows][K], box {32, 32}
+    CUtensorMap map_big128;  // big operand [rows][K], box {32, 128}: a whole tile per TMA (fp32 path)
     CUtensorMap map_small_hi;// small operand [Bpad][K], box {32, n_mma}
     CUtensorMap map_small_lo;
     const TcUnit* units;     // device

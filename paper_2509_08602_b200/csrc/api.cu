@@ -85,7 +85,7 @@ void build_units_k1(int64_t N, int64_t n, int sm, std::vector<TcUnit>& units, st
     double total = 0;
     for (int mt = 0; mt < m_tiles; ++mt) {
         int rows = (int)std::min<int64_t>(kTileM, n - (int64_t)mt * kTileM);
-        cost[mt] = (double)cdiv(rows, kBoxRows) + 2.0;      // A boxes + the small operand, per k-block
+        (void)rows; cost[mt] = 1.0;      // MMA-bound: a partial m-tile costs the same UMMA time per k-block as a full one
         total += cost[mt] * KB;
     }
     const int grid = (int)std::min<int64_t>(sm, (int64_t)m_tiles * std::max<int64_t>(1, KB / 8));
@@ -176,7 +176,9 @@ int chunk_kb(const admm_handle* h) {
     return h->opt.drain_kb > 0 ? h->opt.drain_kb : 1;
 }
 // plans per contraction pass
-int max_pass(const admm_handle* h) { return chunk_kb(h) > 0 ? 128 : kMaxMmaN; }
+int max_pass(const admm_handle* h) {
+    return (mma_passes(h) == 3 && h->opt.kernel_path == ADMM_PATH_TCGEN05) ? 96 : kMaxMmaN;
+}
 
 // one contraction pass over slots [slot0, slot0 + nact): big operand + small hi/lo rows starting at slot0
 admm_status contract(admm_handle* h, int epi, int slot0, int nact, const float* small_hi, const float* small_lo,
@@ -186,6 +188,7 @@ admm_status contract(admm_handle* h, int epi, int slot0, int nact, const float* 
     const bool k1 = (epi == EPI_K1_PARTIAL);
     const int64_t big_rows = k1 ? h->n : h->N, big_cols = k1 ? h->N : h->n, big_ld = k1 ? h->ldN : h->ldn;
     ST_TRY(tc_make_map(h, &L.map_big, k1 ? h->d_phiT : h->d_phi, big_rows, big_cols, big_ld, kBoxRows));
+    ST_TRY(tc_make_map(h, &L.map_big128, k1 ? h->d_phiT : h->d_phi, big_rows, big_cols, big_ld, kTileM));
     // the small operand has Bpad rows allocated; rows >= nact of the box are dead columns of D
     ST_TRY(tc_make_map(h, &L.map_small_hi, small_hi + (int64_t)slot0 * big_ld, h->Bpad - slot0, big_cols, big_ld, n_mma));
     ST_TRY(tc_make_map(h, &L.map_small_lo, small_lo + (int64_t)slot0 * big_ld, h->Bpad - slot0, big_cols, big_ld, n_mma));
@@ -681,7 +684,7 @@ admm_status admm_solve_batch(admm_handle* h, int32_t B, const float* weights, co
 
 admm_status admm_contract_probe(admm_handle* h, int32_t which, int32_t B, const float* small, double* out) {
     if (!h || !small || !out) return ADMM_EINVAL;
-    if (B < 1 || B > max_pass(h) || (which != 0 && which != 1)) { h->err = "probe: need 1 <= B <= 128 (fp32 path) / 256, which in {0,1}"; return ADMM_EINVAL; }
+    if (B < 1 || B > max_pass(h) || (which != 0 && which != 1)) { h->err = "probe: need 1 <= B <= 96 (fp32 path) / 256, which in {0,1}"; return ADMM_EINVAL; }
     CU_TRY(h, cudaSetDevice(h->opt.device));
     cudaStream_t st = h->stream;
     ST_TRY(ensure_batch_buffers(h, B));

@@ -55,36 +55,39 @@ struct EpiCtx {
 };
 
 // 16 consecutive columns c0..c0+15 of this thread's row: q[jj] = accumulator of plan (slot0 + c0 + jj).
-__device__ __forceinline__ void epi_cols16(const TcLaunch& L, const EpiCtx& cx, int c0, const float* q) {
+// Deliberately NOT inlined and with a rolled column loop (q, so, mw live in local memory): unrolled it is ~6000
+// instructions per call site and the unit epilogue then runs at instruction-cache-miss speed (ncu: stall_no_inst).
+__device__ __noinline__ void epi_cols16(const TcLaunch& L, const EpiCtx& cx, int c0, const float* q) {
     const EpiParams& ep = L.ep;
     const int n_act = ep.n_slots_active;
-    if (L.epi == EPI_K1_PARTIAL) {
+    const int epi = L.epi;
+    if (epi == EPI_K1_PARTIAL) {
         float* dst = ep.partial + ((int64_t)cx.slot * ep.n_mma) * kTileM + cx.lrow;
-#pragma unroll
+#pragma unroll 4
         for (int jj = 0; jj < 16; ++jj)
             if (c0 + jj < n_act) dst[(int64_t)(c0 + jj) * kTileM] = q[jj];
         return;
     }
-    if (L.epi == EPI_RAW) {
-#pragma unroll
+    if (epi == EPI_RAW) {
+#pragma unroll 4
         for (int jj = 0; jj < 16; ++jj)
             if (c0 + jj < n_act && cx.valid) ep.qraw[(int64_t)(ep.slot0 + c0 + jj) * ep.ldN + cx.row] = q[jj];
         return;
     }
     float so[16];
     uint32_t mw[16];
-    if (cx.valid) {
+    // all loads of the 16 columns first (one DRAM latency instead of sixteen)
 #pragma unroll
-        for (int jj = 0; jj < 16; ++jj) {
-            const int p = c0 + jj;
-            so[jj] = 0.0f; mw[jj] = 0xFFFFFFFFu;
-            if (p < n_act) {
-                if (L.epi == EPI_K3_STATE) so[jj] = ep.s1[(int64_t)(ep.slot0 + p) * ep.ldN + cx.row];
-                if (ep.mask) mw[jj] = __ldg(ep.mask + (int64_t)__ldg(ep.slot_plan + ep.slot0 + p) * ep.mask_words + cx.mword);
-            }
+    for (int jj = 0; jj < 16; ++jj) {
+        const int p = c0 + jj;
+        float sv = 0.0f; uint32_t m = 0xFFFFFFFFu;
+        if (cx.valid && p < n_act) {
+            if (epi == EPI_K3_STATE) sv = ep.s1[(int64_t)(ep.slot0 + p) * ep.ldN + cx.row];
+            if (ep.mask) m = __ldg(ep.mask + (int64_t)__ldg(ep.slot_plan + ep.slot0 + p) * ep.mask_words + cx.mword);
         }
+        so[jj] = sv; mw[jj] = m;
     }
-#pragma unroll
+#pragma unroll 1
     for (int jj = 0; jj < 16; ++jj) {
         const int p = c0 + jj;
         if (p >= n_act) break;                      // warp-uniform
@@ -92,7 +95,7 @@ __device__ __forceinline__ void epi_cols16(const TcLaunch& L, const EpiCtx& cx, 
         float hinge = 0.f;
         if (cx.valid) {
             const bool on = (mw[jj] >> (cx.row & 31)) & 1u;
-            if (L.epi == EPI_K3_STATE) {
+            if (epi == EPI_K3_STATE) {
                 const float ub = on ? __ldg(ep.utab + cx.cls * kMaxBpad + ep.slot0 + p) : 0.0f;
                 const float cr = __ldg(ep.crtab + cx.cls * kMaxBpad + ep.slot0 + p);
                 Epi1Out o = epi1_element(so[jj], q[jj], cx.a_k, cr, ub, cx.resid, racc);
@@ -110,7 +113,8 @@ __device__ __forceinline__ void epi_cols16(const TcLaunch& L, const EpiCtx& cx, 
                 float v = warp_sum(racc[t]);
                 if (cx.lane == 0) cx.wacc[p * 8 + t] += v;
             }
-        } else if (L.epi == EPI_OBJECTIVE) {
+        } else if (epi == EPI_OBJECTIVE) {
+#pragma unroll 1
             for (int k = 0; k < kMaxClasses; ++k) {
                 float v = warp_sum((cx.valid && cx.cls == k) ? hinge : 0.0f);
                 if (cx.lane == 0) cx.wacc[p * 8 + k] += v;
@@ -394,6 +398,463 @@ __global__ void __launch_bounds__(DRAIN ? 448 : 320, 1) admm_contract_kernel(con
     }
 }
 
+
+// Epilogue of one unit from a staged accumulator tile qs[col][128 rows] in shared memory (written by the drain warps).
+// One warp = 32 consecutive rows (lane = row), a loop over the plans in batches of 16 whose s1 loads are all in flight
+// together; it runs concurrently with the MMAs / drains of the next unit.  Specialised at compile time on the epilogue
+// kind and on whether residual sums are wanted: the hot instance (K3, no residuals) is ~40 instructions per plan (an
+// earlier all-in-one version was instruction-fetch bound).  wacc: this warp's [n_mma][8] partial sums.
+// Pull the s1 tile of a unit into L2 long before its epilogue needs it (the epilogue warps are otherwise exposed to
+// the loaded HBM latency once per batch of plans).
+__device__ __forceinline__ void prefetch_s1_tile(const TcLaunch& L, const TcUnit& un, int wq, int lane, int p_begin, int p_end) {
+    const EpiParams& ep = L.ep;
+    const int lrow = wq * 32 + lane;
+    if (L.epi != EPI_K3_STATE || lrow >= un.rows) return;
+    const float* s1p = ep.s1 + (int64_t)ep.slot0 * ep.ldN + un.row0 + lrow;
+    for (int p = p_begin; p < p_end; ++p)
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(s1p + (int64_t)p * ep.ldN));
+}
+
+// Epilogue of one unit from a staged accumulator tile qs[col][128 rows] in shared memory (written by the drain warps).
+// One warp = 32 consecutive rows (lane = row) x the plans [p_begin, p_end), in batches of 8 whose loads are all in
+// flight together; it runs concurrently with the MMAs / drains of the next unit.  Specialised at compile time on the
+// epilogue kind and on whether residual sums are wanted, 32-bit element offsets: the hot instance (K3, no residuals,
+// no mask) is ~35 instructions per plan (an all-in-one version was instruction-fetch and issue bound).
+// wacc: this warp's [n_mma][8] partial sums.
+template <int EPI, bool RESID>
+__device__ __noinline__ void epilogue_unit_t(const TcLaunch& L, const TcUnit& un, const float* qs, int wq, int lane, float* wacc,
+                                             int p_begin, int p_end) {
+    const EpiParams& ep = L.ep;
+    const int lrow = wq * 32 + lane;
+    const bool valid = lrow < un.rows;
+    const int64_t row = (int64_t)un.row0 + lrow;
+    const float* qp = qs + lrow;
+    if (EPI == EPI_K1_PARTIAL) {
+        float* dst = ep.partial + ((int64_t)un.slot * ep.n_mma) * kTileM + lrow;
+#pragma unroll 8
+        for (int p = p_begin; p < p_end; ++p) dst[p * kTileM] = qp[p * kTileM];
+        return;
+    }
+    if (EPI == EPI_RAW) {
+        if (valid) {
+            float* dst = ep.qraw + (int64_t)ep.slot0 * ep.ldN + row;
+#pragma unroll 8
+            for (int p = p_begin; p < p_end; ++p) dst[(int64_t)p * ep.ldN] = qp[p * kTileM];
+        }
+        return;
+    }
+    const int cls = valid ? ep.point_class[row] : 0;
+    const float a_k = ep.a_cls[cls], sense = ep.sense[cls], thr = ep.thr[cls];
+    const uint32_t mbit = (uint32_t)(row & 31);
+    const float* utab = ep.utab + cls * kMaxBpad + ep.slot0;
+    const float* crtab = ep.crtab + cls * kMaxBpad + ep.slot0;
+    const int32_t* splan = ep.slot_plan + ep.slot0;
+    const uint32_t* mrow = ep.mask ? ep.mask + (row >> 5) : nullptr;
+    const uint32_t ldN = (uint32_t)ep.ldN;                     // Bpad * ldN < 2^32 (checked on the host)
+    const int64_t base = (int64_t)ep.slot0 * ep.ldN + row;
+    float* s1p = ep.s1 + base;
+    float* ghp = ep.g_hi + base;
+    float* glp = ep.g_lo + base;
+    constexpr int PB = 8;
+    for (int p0 = p_begin; p0 < p_end; p0 += PB) {
+        float so[PB], ub[PB], cr[PB];
+        uint32_t mw[PB];
+#pragma unroll
+        for (int j = 0; j < PB; ++j) {
+            const int p = p0 + j;
+            const bool live = valid && p < p_end;
+            so[j] = 0.f; ub[j] = 0.f; cr[j] = 0.f; mw[j] = 0xFFFFFFFFu;
+            if (live) {
+                if (EPI == EPI_K3_STATE) { so[j] = s1p[(uint32_t)p * ldN]; ub[j] = __ldg(utab + p); cr[j] = __ldg(crtab + p); }
+                if (mrow) mw[j] = __ldg(mrow + (int64_t)__ldg(splan + p) * ep.mask_words);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < PB; ++j) {
+            const int p = p0 + j;
+            if (p >= p_end) break;                      // warp-uniform
+            float racc[kNumResid] = {0.f, 0.f, 0.f, 0.f, 0.f};
+            float hinge = 0.f;
+            if (valid) {
+                const bool on = (mw[j] >> mbit) & 1u;
+                const float q = qp[p * kTileM];
+                if (EPI == EPI_K3_STATE) {
+                    Epi1Out o = epi1_element(so[j], q, a_k, cr[j], on ? ub[j] : 0.0f, RESID, racc);
+                    const uint32_t off = (uint32_t)p * ldN;
+                    s1p[off] = o.s_new;
+                    ghp[off] = o.g_hi;
+                    glp[off] = o.g_lo;
+                } else {
+                    hinge = on ? fmaxf(0.0f, sense * (thr - q)) : 0.0f;
+                }
+            }
+            if (EPI == EPI_K3_STATE && RESID) {
+#pragma unroll
+                for (int t = 0; t < kNumResid; ++t) {
+                    float v = warp_sum(racc[t]);
+                    if (lane == 0) wacc[p * 8 + t] += v;
+                }
+            } else if (EPI == EPI_OBJECTIVE) {
+#pragma unroll 1
+                for (int k = 0; k < kMaxClasses; ++k) {
+                    float v = warp_sum((valid && cls == k) ? hinge : 0.0f);
+                    if (lane == 0) wacc[p * 8 + k] += v;
+                }
+            }
+        }
+    }
+}
+
+__device__ __forceinline__ void epilogue_unit(const TcLaunch& L, const TcUnit& un, const float* qs, int wq, int lane, float* wacc,
+                                              int p_begin, int p_end) {
+    switch (L.epi) {
+        case EPI_K1_PARTIAL: epilogue_unit_t<EPI_K1_PARTIAL, false>(L, un, qs, wq, lane, wacc, p_begin, p_end); break;
+        case EPI_K3_STATE:
+            if (L.ep.resid_partial != nullptr) epilogue_unit_t<EPI_K3_STATE, true>(L, un, qs, wq, lane, wacc, p_begin, p_end);
+            else epilogue_unit_t<EPI_K3_STATE, false>(L, un, qs, wq, lane, wacc, p_begin, p_end);
+            break;
+        case EPI_OBJECTIVE: epilogue_unit_t<EPI_OBJECTIVE, false>(L, un, qs, wq, lane, wacc, p_begin, p_end); break;
+        default: epilogue_unit_t<EPI_RAW, false>(L, un, qs, wq, lane, wacc, p_begin, p_end); break;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// The fp32 path (ADMM_STORAGE_FP32_3XTF32): 3xTF32 with the big operand split ON CHIP INTO TENSOR MEMORY.
+//
+//   warp 0        TMA producer: raw fp32 tile of the big operand [128 rows][32] + the small operand [hi ; lo] stacked
+//                 as ONE [2 n_mma][32] K-major tile
+//   warps 2-5     converter: thread = one row.  Reads its 128 B from the swizzled smem tile, splits every value into
+//                 hi = tf32_rna(x), lo = tf32_rna(x - hi) and writes both with tcgen05.st into a 2-deep TMEM ring
+//                 (the A operand of the MMAs: lanes = rows, 32 columns = the k-block)
+//   warp 1        UMMA issuer, per 8-element k-step TWO instructions (measured: a tf32 MMA of M=128 costs ~120 cycles
+//                 for any N <= 192, so stacking [hi ; lo] along N is free):
+//                     D[:, 0:2n)  += A_hi . [B_hi ; B_lo]^T      (main | small)
+//                     D[:, n:2n)  += A_lo . B_hi^T               (small)
+//   warps 6-13    drain + epilogue: tcgen05.mma adds with truncation (measured: every product is cut 2 bits below the
+//                 accumulator's ulp and the sum is cut toward zero: a bias of ~0.45 ulp per MMA that is coherent over
+//                 the iterations).  The MAIN accumulator is therefore read AND CLEARED every `chunk_kb` k-blocks and
+//                 summed in fp32 registers with round-to-nearest FADDs; the MMAs always accumulate.  Two D regions
+//                 alternate so the drain of chunk c overlaps the MMAs of chunk c+1.  The small (2^-11) terms stay in
+//                 TMEM for the whole unit.
+// TMEM columns: region 0 [0, 2n) | region 1 [2n, 4n) | A ring [384, 512) = 2 x (hi 32 | lo 32);   n = n_mma <= 96.
+constexpr int kF32Warps = 22;              // TMA, MMA, 4 converter, 8 drain, 8 epilogue
+constexpr int kF32Threads = kF32Warps * 32;
+constexpr int kF32MaxMmaN = 96;
+constexpr int kAcol = 384;
+constexpr int kConvWarp0 = 2, kDrainWarp0 = 6, kEpiWarp0 = 14;    // first warp of each role (4 consecutive warps cover the 4 TMEM lane quarters)
+constexpr int kMaxAStages = 8, kMaxBStages = 4;
+
+struct CtrlF32 {
+    uint64_t sa_full[kMaxAStages];     // raw fp32 tile of the big operand landed in smem      (TMA -> converter)
+    uint64_t sa_empty[kMaxAStages];    // converter has it in registers                         (converter -> TMA)
+    uint64_t sb_full[kMaxBStages];     // small operand [hi ; lo] landed in smem                (TMA -> MMA)
+    uint64_t sb_empty[kMaxBStages];    // MMAs that read it completed                           (MMA commit -> TMA)
+    uint64_t a_full[2];                // hi | lo of a k-block are in TMEM                      (converter -> MMA)
+    uint64_t a_empty[2];               //                                                       (MMA commit -> converter)
+    uint64_t d_full[2];                // a chunk of MMAs into D region a completed             (MMA commit -> drain)
+    uint64_t d_empty[2];               // region read and cleared                               (drain -> MMA)
+    uint64_t q_full;                   // master sums of a unit staged in qs                    (drain -> epilogue)
+    uint64_t q_empty;                  //                                                       (epilogue -> drain)
+    uint32_t tmem_base;
+    uint32_t pad;
+};
+__host__ __device__ inline int f32_b_bytes(int n_mma) { return 2 * n_mma * kBlockK * 4; }
+__host__ __device__ inline int f32_q_bytes(int n_mma) { return n_mma * kTileM * 4; }        // staged accumulator tile
+__host__ __device__ inline int f32_acc_bytes(int n_mma) { return 8 * n_mma * 8 * 4; }       // [8 warps][n_mma][8]
+// B ring: 3 stages (L2-resident operand, short latency); everything left goes to the A ring, whose depth is what
+// keeps enough HBM bytes in flight (ncu: with 4 x 16 KB the converter waited on TMA a third of the time)
+__host__ __device__ inline int f32_b_stages(int) { return 3; }
+__host__ __device__ inline int f32_a_stages(int n_mma) {
+    int s = (kSmemLimit - 1024 - (int)sizeof(CtrlF32) - f32_q_bytes(n_mma) - f32_acc_bytes(n_mma) -
+             f32_b_stages(n_mma) * f32_b_bytes(n_mma)) / kTileBytes;
+    return s > kMaxAStages ? kMaxAStages : s;
+}
+
+// iterator over the (unit, k-block) sequence of this CTA
+struct KbIter {
+    int u, kb, kb_count;
+    __device__ __forceinline__ void start(const TcLaunch& L, int u0, int u_end) {
+        u = u0; kb = 0; kb_count = (u0 < u_end) ? L.units[u0].kb_count : 0;
+    }
+    __device__ __forceinline__ void next(const TcLaunch& L, int u_end) {
+        if (++kb == kb_count) { ++u; kb = 0; kb_count = (u < u_end) ? L.units[u].kb_count : 0; }
+    }
+};
+
+__global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const __grid_constant__ TcLaunch L) {
+    extern __shared__ __align__(1024) uint8_t smem[];
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int n_mma = L.ep.n_mma;
+    const int bbytes = f32_b_bytes(n_mma);
+    const int n_sa = f32_a_stages(n_mma);
+    const int n_sb = f32_b_stages(n_mma);
+    uint8_t* a_ring = smem;                                   // n_sa x 16 KB (1024-aligned)
+    uint8_t* b_ring = smem + n_sa * kTileBytes;               // n_sb x bbytes (multiple of 1024: n_mma % 16 == 0)
+    float* qs = reinterpret_cast<float*>(b_ring + n_sb * bbytes);
+    float* acc = qs + n_mma * kTileM;
+    CtrlF32* ctrl = reinterpret_cast<CtrlF32*>(reinterpret_cast<uint8_t*>(acc) + f32_acc_bytes(n_mma));
+
+    const int unit_begin = L.cta_unit_begin[blockIdx.x];
+    const int unit_end = L.cta_unit_begin[blockIdx.x + 1];
+    const int chunk_kb = L.chunk_kb;
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < n_sa; ++i) { tc::mbar_init(&ctrl->sa_full[i], 1); tc::mbar_init(&ctrl->sa_empty[i], 4); }
+        for (int i = 0; i < n_sb; ++i) { tc::mbar_init(&ctrl->sb_full[i], 1); tc::mbar_init(&ctrl->sb_empty[i], 1); }
+        for (int i = 0; i < 2; ++i) {
+            tc::mbar_init(&ctrl->a_full[i], 4);
+            tc::mbar_init(&ctrl->a_empty[i], 1);
+            tc::mbar_init(&ctrl->d_full[i], 1);
+            tc::mbar_init(&ctrl->d_empty[i], 8);
+        }
+        tc::mbar_init(&ctrl->q_full, 8);
+        tc::mbar_init(&ctrl->q_empty, 8);
+        tc::fence_barrier_init();
+        tc::tma_prefetch_desc(&L.map_big);
+        tc::tma_prefetch_desc(&L.map_small_hi);
+        tc::tma_prefetch_desc(&L.map_small_lo);
+    }
+    for (int i = threadIdx.x; i < f32_acc_bytes(n_mma) / 4; i += kF32Threads) acc[i] = 0.0f;
+    if (warp == 1) tc::tmem_alloc(&ctrl->tmem_base, 512);
+    tc::tcgen05_fence_before();
+    __syncthreads();
+    tc::tcgen05_fence_after();
+    const uint32_t tmem_base = ctrl->tmem_base;
+    if (warp >= kDrainWarp0 && warp < kEpiWarp0) {
+        // the MMAs always accumulate: clear both D regions once (this warp's lane quarter, its half of 384 columns)
+        const uint32_t lane_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
+        uint32_t z[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) z[i] = 0u;
+        const int c_lo = ((warp - kDrainWarp0) >> 2) * (kAcol / 2);
+        for (int c = c_lo; c < c_lo + kAcol / 2; c += 16) tc::tmem_st16(lane_addr + c, z);
+        tc::tmem_st_wait();
+    }
+    tc::tcgen05_fence_before();
+    __syncthreads();
+    tc::tcgen05_fence_after();
+
+    if (warp == 0) {
+        // ------------------------------------------------------------ TMA producer: two independent rings, one polling lane
+        if (lane == 0) {
+            KbIter ia, ib;
+            ia.start(L, unit_begin, unit_end); ib.start(L, unit_begin, unit_end);
+            int sa = 0, sb = 0; uint32_t pha = 0, phb = 0;
+            while (ia.u < unit_end || ib.u < unit_end) {
+                if (ia.u < unit_end && tc::mbar_test_wait(&ctrl->sa_empty[sa], pha ^ 1)) {
+                    const TcUnit un = L.units[ia.u];
+                    // one 128-row box: rows past the end of the matrix are zero-filled by TMA, rows past the end of the
+                    // unit belong to a neighbouring unit and are ignored by the epilogue
+                    tc::mbar_arrive_expect_tx(&ctrl->sa_full[sa], kTileBytes);
+                    tc::tma_load_2d(a_ring + sa * kTileBytes, &L.map_big128, &ctrl->sa_full[sa], (un.kb0 + ia.kb) * kBlockK,
+                                    un.row0, tc::kEvictFirst);
+                    ia.next(L, unit_end);
+                    if (++sa == n_sa) { sa = 0; pha ^= 1; }
+                }
+                if (ib.u < unit_end && tc::mbar_test_wait(&ctrl->sb_empty[sb], phb ^ 1)) {
+                    const int k0 = (L.units[ib.u].kb0 + ib.kb) * kBlockK;
+                    tc::mbar_arrive_expect_tx(&ctrl->sb_full[sb], bbytes);
+                    tc::tma_load_2d(b_ring + sb * bbytes, &L.map_small_hi, &ctrl->sb_full[sb], k0, 0, tc::kEvictLast);
+                    tc::tma_load_2d(b_ring + sb * bbytes + bbytes / 2, &L.map_small_lo, &ctrl->sb_full[sb], k0, 0, tc::kEvictLast);
+                    ib.next(L, unit_end);
+                    if (++sb == n_sb) { sb = 0; phb ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ------------------------------------------------------------ UMMA issuer (warp-uniform loop, one elected lane issues)
+        const uint32_t idesc_wide = tc::umma_idesc(2u, kTileM, (uint32_t)(2 * n_mma));
+        const uint32_t idesc_one = tc::umma_idesc(2u, kTileM, (uint32_t)n_mma);
+        const uint64_t b_desc0 = tc::umma_desc_k_sw128(tc::smem_u32(b_ring));
+        const uint64_t b_step = (uint64_t)(bbytes >> 4);
+        uint64_t b_desc = b_desc0;
+        int sb = 0; uint32_t phb = 0;      // smem B ring
+        int t = 0; uint32_t tph = 0;       // TMEM A ring
+        int a = 0; uint32_t aph = 0;       // D region
+        for (int u = unit_begin; u < unit_end; ++u) {
+            const int kb_count = L.units[u].kb_count;
+            const int ck = chunk_kb > 0 ? chunk_kb : kb_count;
+            for (int kb0 = 0; kb0 < kb_count; kb0 += ck) {
+                const int nkb = min(ck, kb_count - kb0);
+                tc::mbar_wait(&ctrl->d_empty[a], aph ^ 1);
+                const uint32_t d_main = tmem_base + a * 2 * n_mma;
+                const uint32_t d_small = d_main + n_mma;
+                for (int kb = 0; kb < nkb; ++kb) {
+                    tc::mbar_wait(&ctrl->sb_full[sb], phb);     // the small operand landed (async proxy)
+                    tc::mbar_wait(&ctrl->a_full[t], tph);       // the converter's hi/lo are in TMEM
+                    tc::tcgen05_fence_after();
+                    const uint32_t a_hi = tmem_base + kAcol + t * 64;
+                    if (tc::elect_one()) {
+#pragma unroll
+                        for (int k = 0; k < kBlockK / 8; ++k) {
+                            tc::umma_tf32_ts(d_main, a_hi + k * 8, b_desc + 2 * k, idesc_wide, 1u);
+                            tc::umma_tf32_ts(d_small, a_hi + 32 + k * 8, b_desc + 2 * k, idesc_one, 1u);
+                        }
+                        tc::umma_commit(&ctrl->sb_empty[sb]);
+                        tc::umma_commit(&ctrl->a_empty[t]);
+                        if (kb == nkb - 1) tc::umma_commit(&ctrl->d_full[a]);
+                    }
+                    __syncwarp();
+                    b_desc += b_step;
+                    if (++sb == n_sb) { sb = 0; phb ^= 1; b_desc = b_desc0; }
+                    if (++t == 2) { t = 0; tph ^= 1; }
+                }
+                if (++a == 2) { a = 0; aph ^= 1; }
+            }
+        }
+    } else if (warp >= kConvWarp0 && warp < kDrainWarp0) {
+        // ------------------------------------------------------------ converter: smem fp32 row -> TMEM hi | lo
+        // hi = tf32_rna(x) (round to nearest: lo = x - hi is then symmetric in sign, so the tensor core's truncation of
+        // lo's low bits is unbiased; with a truncated hi, lo >= 0 for Phi >= 0 and the products came out 2^-22 too small)
+        const int q = warp & 3;                         // TMEM lane quarter of this warp
+        const int lrow = q * 32 + lane;
+        const uint32_t lane_addr = tmem_base + ((uint32_t)(q * 32) << 16) + kAcol;
+        int sa = 0; uint32_t pha = 0;
+        int t = 0; uint32_t tph = 0;
+        for (int u = unit_begin; u < unit_end; ++u) {
+            const int kbc = L.units[u].kb_count;
+            for (int kb = 0; kb < kbc; ++kb) {
+                tc::mbar_wait(&ctrl->sa_full[sa], pha);
+                const uint8_t* row = a_ring + sa * kTileBytes + lrow * 128;
+                float4 v[8];
+#pragma unroll
+                for (int c = 0; c < 8; ++c) v[c] = *reinterpret_cast<const float4*>(row + ((c ^ (lrow & 7)) << 4));
+                __syncwarp();
+                if (lane == 0) tc::mbar_arrive(&ctrl->sa_empty[sa]);      // the raw tile is in registers: free the slot
+                tc::mbar_wait(&ctrl->a_empty[t], tph ^ 1);
+                tc::tcgen05_fence_after();
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    uint32_t hi[16], lo[16];
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        const float4 x = v[h * 4 + c];
+                        const float xs[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            const float hf = tc::tf32_rna(xs[e]);
+                            hi[c * 4 + e] = __float_as_uint(hf);
+                            lo[c * 4 + e] = __float_as_uint(xs[e] - hf);
+                        }
+                    }
+                    tc::tmem_st16(lane_addr + t * 64 + h * 16, hi);
+                    tc::tmem_st16(lane_addr + t * 64 + 32 + h * 16, lo);
+                }
+                tc::tmem_st_wait();
+                tc::tcgen05_fence_before();
+                __syncwarp();
+                if (lane == 0) tc::mbar_arrive(&ctrl->a_full[t]);
+                if (++sa == n_sa) { sa = 0; pha ^= 1; }
+                if (++t == 2) { t = 0; tph ^= 1; }
+            }
+        }
+    } else if (warp >= kDrainWarp0 && warp < kEpiWarp0) {
+        // ------------------------------------------------------------ drain (row = TMEM lane): TMEM -> fp32 master sums -> qs
+        const int ew = warp & 3;
+        const int n16 = n_mma / 16;
+        const int half = (warp - kDrainWarp0) >> 2;
+        const int cbeg = half == 0 ? 0 : (n16 + 1) / 2;          // first 16-column group of this warp
+        const int cend = half == 0 ? (n16 + 1) / 2 : n16;        // at most 3 groups (n_mma <= 96)
+        const int lrow = ew * 32 + lane;
+        const uint32_t lane_addr = tmem_base + ((uint32_t)(ew * 32) << 16);
+        uint32_t zero[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) zero[i] = 0u;
+        int a = 0; uint32_t aph = 0;
+        uint32_t qph = 0;
+        for (int u = unit_begin; u < unit_end; ++u) {
+            const int kb_count = L.units[u].kb_count;
+            float master[48];
+#pragma unroll
+            for (int i = 0; i < 48; ++i) master[i] = 0.0f;
+            const int ck = chunk_kb > 0 ? chunk_kb : kb_count;
+            const int nchunks = (kb_count + ck - 1) / ck;
+            for (int ci = 0; ci < nchunks; ++ci) {
+                tc::mbar_wait(&ctrl->d_full[a], aph);
+                tc::tcgen05_fence_after();
+                const uint32_t d_main = lane_addr + a * 2 * n_mma;
+                const bool with_small = ci + 2 >= nchunks;       // last use of this region in the unit
+#pragma unroll
+                for (int cc = 0; cc < 3; ++cc) {
+                    if (cbeg + cc < cend) {
+                        uint32_t r[16];
+                        tc::tmem_ld16(d_main + (cbeg + cc) * 16, r);
+                        tc::tmem_ld_wait(r);
+#pragma unroll
+                        for (int jj = 0; jj < 16; ++jj) master[cc * 16 + jj] += __uint_as_float(r[jj]);
+                        tc::tmem_st16(d_main + (cbeg + cc) * 16, zero);
+                        if (with_small) {
+                            tc::tmem_ld16(d_main + n_mma + (cbeg + cc) * 16, r);
+                            tc::tmem_ld_wait(r);
+#pragma unroll
+                            for (int jj = 0; jj < 16; ++jj) master[cc * 16 + jj] += __uint_as_float(r[jj]);
+                            tc::tmem_st16(d_main + n_mma + (cbeg + cc) * 16, zero);
+                        }
+                    }
+                }
+                tc::tmem_st_wait();
+                tc::tcgen05_fence_before();
+                __syncwarp();
+                if (lane == 0) tc::mbar_arrive(&ctrl->d_empty[a]);
+                if (++a == 2) { a = 0; aph ^= 1; }
+            }
+            // hand the finished tile to the epilogue warps and go on draining the next unit
+            tc::mbar_wait(&ctrl->q_empty, qph ^ 1);
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) {
+                if (cbeg + cc < cend) {
+#pragma unroll
+                    for (int jj = 0; jj < 16; ++jj) qs[((cbeg + cc) * 16 + jj) * kTileM + lrow] = master[cc * 16 + jj];
+                }
+            }
+            __syncwarp();
+            if (lane == 0) tc::mbar_arrive(&ctrl->q_full);
+            qph ^= 1;
+        }
+    } else if (warp >= kEpiWarp0) {
+        // ------------------------------------------------------------ epilogue warps: qs -> global, concurrent with the next unit
+        const int wq = (warp - kEpiWarp0) & 3;           // row quarter
+        const int ph_half = (warp - kEpiWarp0) >> 2;     // which half of the plans
+        const int n_act = L.ep.n_slots_active;
+        const int p_mid = (n_act + 1) / 2;
+        const int p_begin = ph_half == 0 ? 0 : p_mid;
+        const int p_end = ph_half == 0 ? p_mid : n_act;
+        uint32_t qph = 0;
+        if (unit_begin < unit_end) prefetch_s1_tile(L, L.units[unit_begin], wq, lane, p_begin, p_end);
+        for (int u = unit_begin; u < unit_end; ++u) {
+            const TcUnit un = L.units[u];
+            if (u + 1 < unit_end) prefetch_s1_tile(L, L.units[u + 1], wq, lane, p_begin, p_end);
+            tc::mbar_wait(&ctrl->q_full, qph);
+            epilogue_unit(L, un, qs, wq, lane, acc + (warp - kEpiWarp0) * n_mma * 8, p_begin, p_end);
+            __syncwarp();
+            if (lane == 0) tc::mbar_arrive(&ctrl->q_empty);
+            qph ^= 1;
+        }
+    }
+
+    __syncthreads();
+    if (L.epi == EPI_K3_STATE && L.ep.resid_partial != nullptr) {
+        for (int i = threadIdx.x; i < L.ep.n_slots_active * kNumResid; i += kF32Threads) {
+            const int p = i / kNumResid, t = i % kNumResid;
+            float v = 0.f;
+            for (int w = 0; w < 8; ++w) v += acc[(w * n_mma + p) * 8 + t];
+            L.ep.resid_partial[((int64_t)blockIdx.x * kMaxBpad + L.ep.slot0 + p) * kNumResid + t] = v;
+        }
+    } else if (L.epi == EPI_OBJECTIVE) {
+        for (int i = threadIdx.x; i < L.ep.n_slots_active * kMaxClasses; i += kF32Threads) {
+            const int p = i / kMaxClasses, k = i % kMaxClasses;
+            double v = 0.0;
+            for (int w = 0; w < 8; ++w) v += (double)acc[(w * n_mma + p) * 8 + k];
+            L.ep.hinge_partial[((int64_t)blockIdx.x * kMaxBpad + L.ep.slot0 + p) * kMaxClasses + k] = v;
+        }
+    }
+    if (warp == 1) {
+        tc::tcgen05_fence_after();
+        tc::tmem_dealloc(tmem_base, 512);
+    }
+}
+
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -412,7 +873,7 @@ admm_status tc_init(admm_handle* h) {
         }
         g_encode = reinterpret_cast<EncodeTiledFn>(fn);
     }
-    cudaError_t e = cudaFuncSetAttribute(admm_contract_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+    cudaError_t e = cudaFuncSetAttribute(admm_contract_f32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(admm_contract_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
     if (e != cudaSuccess) {
         h->err = std::string("cudaFuncSetAttribute(max dynamic smem): ") + cudaGetErrorString(e);
@@ -454,9 +915,10 @@ admm_status tc_launch(admm_handle* h, const TcLaunch& L) {
         h->err = "tc_launch: fewer than 2 pipeline stages fit in shared memory";
         return ADMM_EINVAL;
     }
-    if (L.chunk_kb > 0) {
-        if (n_mma > 128) { h->err = "tc_launch: the drained (fp32) path needs n_mma <= 128"; return ADMM_EINVAL; }
-        admm_contract_kernel<true><<<L.grid, 448, kSmemLimit, h->stream>>>(L);
+    if (L.mma_passes == 3) {
+        if (n_mma > kF32MaxMmaN) { h->err = "tc_launch: the fp32 path needs n_mma <= 96"; return ADMM_EINVAL; }
+        if (f32_a_stages(n_mma) < 2) { h->err = "tc_launch: fewer than 2 pipeline stages fit in shared memory"; return ADMM_EINVAL; }
+        admm_contract_f32_kernel<<<L.grid, kF32Threads, kSmemLimit, h->stream>>>(L);
     } else {
         admm_contract_kernel<false><<<L.grid, 320, kSmemLimit, h->stream>>>(L);
     }

@@ -53,7 +53,7 @@ def test_contractions_match_fp64_matmul(b, shape):
     rng = np.random.default_rng(1)
     P = w.phi.astype(np.float64)
     h = b.admm_setup(w.phi, w.point_class, w.classes)
-    for which, Bp in ((1, 9), (0, 16), (1, 81), (0, 81), (1, 128)):
+    for which, Bp in ((1, 9), (0, 16), (1, 81), (0, 81), (1, 96)):
         K = w.N if which == 0 else w.n
         small = rng.standard_normal((Bp, K)).astype(np.float32)
         got = b.admm_contract_probe(h, which, small)
@@ -104,7 +104,7 @@ def test_fixed_k_parity_row_masks_multitarget(b):
 
 
 def test_fixed_k_parity_more_than_one_pass_of_plans(b):
-    """B = 144 > 128: the fp32 path runs the contractions in two passes over the plans."""
+    """B = 144 > 96: the fp32 path runs the contractions in two passes over the plans."""
     from workloads import default_rho, make_workload
     w = make_workload(0, n_target=600, n_lowdose=1200, n_iso=4, grid=12)
     ez, ey, et, _, _, _ = _parity(b, w, default_rho(w.beta), 30)

@@ -91,7 +91,9 @@ struct admm_handle {
     float* d_phiT = nullptr;       // [n][ldN]
     uint8_t* d_point_class = nullptr;
     double* d_R = nullptr;         // [n]
-    double* d_Sinv = nullptr;      // [n][n]
+    double* d_Sinv = nullptr;      // [n][lds], lds = n rounded up to even (16-byte rows for cp.async), pad = 0
+    int64_t lds = 0;
+    int k2_wj = 1;                 // K2b block tile = 16 * k2_wj rows (chosen when the batch buffers are allocated)
     std::vector<double> h_R;
 
     // per-solve state (reallocated when B grows)
@@ -153,5 +155,6 @@ void launch_objective_reduce(admm_handle* h, int B, int grid, const float* t_f32
 void launch_gather_rows(const float* src, int64_t ld, const int32_t* plan_slot, int B, int64_t n, float* dst, cudaStream_t s);
 void launch_state_out(admm_handle* h, const EpiParams& ep, int slot, double beta, float* z1, float* y1, double* z2, double* y2, cudaStream_t s);
 int k2b_grid(const admm_handle* h, int Bact);
+int k2_choose_wj(const admm_handle* h, int Bpad);
 void launch_split_tf32(const float* x, int64_t count, float* hi, float* lo, cudaStream_t s);
 void launch_reduce_partial(admm_handle* h, int nact, int n_mma, double* out, cudaStream_t s);

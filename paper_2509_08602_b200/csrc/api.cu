@@ -327,6 +327,16 @@ static admm_status setup_impl(admm_handle* h, const float* phi, int32_t phi_on_d
     if (s1 != CUSOLVER_STATUS_SUCCESS || s2 != CUSOLVER_STATUS_SUCCESS) { h->err = "cuSOLVER potrf/potri failed"; return ADMM_ECUDA; }
     if (info1 != 0 || info2 != 0) { h->err = "S = I + A A^T is not positive definite (non-finite Phi?)"; return ADMM_ENOTSPD; }
     launch_symmetrize(h->d_Sinv, n, st);
+    h->lds = round_up(n, 2);
+    if (h->lds != n) {               // odd n: re-pitch so every row starts 16-byte aligned (K2b stages it with cp.async)
+        double* padded = nullptr;
+        ST_TRY(dev_alloc(h, &padded, n * h->lds));
+        CU_TRY(h, cudaMemsetAsync(padded, 0, (size_t)n * h->lds * 8, st));
+        CU_TRY(h, cudaMemcpy2DAsync(padded, (size_t)h->lds * 8, h->d_Sinv, (size_t)n * 8, (size_t)n * 8, (size_t)n, cudaMemcpyDeviceToDevice, st));
+        CU_TRY(h, cudaStreamSynchronize(st));
+        cudaFree(h->d_Sinv);
+        h->d_Sinv = padded;
+    }
     h->h_R.resize(n);
     CU_TRY(h, cudaMemcpyAsync(h->h_R.data(), h->d_R, (size_t)n * 8, cudaMemcpyDeviceToHost, st));
     CU_TRY(h, cudaStreamSynchronize(st));
@@ -406,11 +416,13 @@ static admm_status ensure_batch_buffers(admm_handle* h, int B) {
     const int Bpad = (int)round_up(B, 16);
     if (Bpad <= h->Bpad && h->d_s1) return ADMM_OK;
     const bool simt = h->opt.kernel_path == ADMM_PATH_SIMT;
+    h->k2_wj = k2_choose_wj(h, Bpad);
     ST_TRY(dev_alloc(h, &h->d_s1, (int64_t)Bpad * h->ldN));
     ST_TRY(dev_alloc(h, &h->d_ghi, (int64_t)Bpad * h->ldN));
     ST_TRY(dev_alloc(h, &h->d_glo, (int64_t)Bpad * h->ldN));
     ST_TRY(dev_alloc(h, &h->d_s2, (int64_t)Bpad * h->ldn));
     ST_TRY(dev_alloc(h, &h->d_rhs, (int64_t)Bpad * h->ldn));
+    CU_TRY(h, cudaMemsetAsync(h->d_rhs, 0, (size_t)Bpad * h->ldn * 8, h->stream));   // pad columns are read (x 0) by K2b
     ST_TRY(dev_alloc(h, &h->d_vhi, (int64_t)Bpad * h->ldn));
     ST_TRY(dev_alloc(h, &h->d_vlo, (int64_t)Bpad * h->ldn));
     ST_TRY(dev_alloc(h, &h->d_partial, (int64_t)h->slots_k1 * std::min(Bpad, max_pass(h)) * kTileM));
@@ -758,7 +770,7 @@ admm_status admm_get_preconditioner(admm_handle* h, double* D, double* R, double
     CU_TRY(h, cudaSetDevice(h->opt.device));
     if (D) for (int64_t i = 0; i < h->N; ++i) D[i] = 1.0 / (double)h->class_count[h->h_point_class[i]];
     if (R) memcpy(R, h->h_R.data(), (size_t)h->n * 8);
-    if (Sinv) CU_TRY(h, cudaMemcpy(Sinv, h->d_Sinv, (size_t)h->n * h->n * 8, cudaMemcpyDeviceToHost));
+    if (Sinv) CU_TRY(h, cudaMemcpy2D(Sinv, (size_t)h->n * 8, h->d_Sinv, (size_t)h->lds * 8, (size_t)h->n * 8, (size_t)h->n, cudaMemcpyDeviceToHost));
     return ADMM_OK;
 }
 

@@ -23,8 +23,8 @@ __device__ __forceinline__ Epi1Out epi1_element(float s_old, float q, float a, f
     float g = a * (2.0f * z_new - s_new - cr);
     Epi1Out o;
     o.s_new = s_new;
-    o.g_hi = tc::tf32_rn(g);
-    o.g_lo = g - o.g_hi;
+    o.g_hi = tc::tf32_rna(g);
+    o.g_lo = tc::tf32_rna(g - o.g_hi);      // rounded here: the tensor core would otherwise cut lo's low bits toward zero
     if (resid) {
         float y_old = s_old - z_old;
         float y_new = s_new - z_new;

@@ -100,9 +100,9 @@ __global__ void emit_g_kernel(const EpiParams ep, int Bact) {
     float s = ep.s1[(int64_t)p * ep.ldN + i];
     float z = fminf(fmaxf(s, 0.f), ub);
     float g = ep.a_cls[cls] * (2.f * z - s - cr);
-    float hi = tc::tf32_rn(g);
+    float hi = tc::tf32_rna(g);
     ep.g_hi[(int64_t)p * ep.ldN + i] = hi;
-    ep.g_lo[(int64_t)p * ep.ldN + i] = g - hi;
+    ep.g_lo[(int64_t)p * ep.ldN + i] = tc::tf32_rna(g - hi);
 }
 
 __global__ void state_out_kernel(const EpiParams ep, int slot, const double* __restrict__ s2, const double* __restrict__ R,
@@ -159,110 +159,164 @@ __global__ void k2a_kernel(const float* __restrict__ partial, const int32_t* __r
 }
 
 // ------------------------------------------------------------------------------------------ K2b: v = S^-1 rhs + epilogue-2
-// Tile: 32 plans x 32 columns per block of 128 threads (each thread 2 plans x 4 columns), k-chunks of 16.
+// Eq. (6): v = S^-1 (A r1 - r2) with the explicit fp64 inverse computed once at setup (:91, :165).
+// fp64 on purpose (SURVEY H-a): this product is ~1 % of the flops of an iteration and its
+// rounding error, amplified by cond(S), is what dominates the iterate error when it is done in fp32.
+// tcgen05 has no fp64 kind; the fp64 tensor path of sm_100 is mma.sync m8n8k4 (DMMA), used here directly.
+//
+// Block = WJ x 2 warps; warp tile = 16 rows (time variables j) x 48 plans = 2 x 6 DMMA fragments; block tile = 16 WJ x 96.
+// K is walked in chunks of 32 through a 3-stage cp.async ring; both operands are K-contiguous in memory
+// (Sinv[j][k] row-major with padded row stride, rhs[p][k] plan-major), rows padded to 36 doubles => conflict-free LDS.64.
 // Epilogue (4b)/(4c) on block 2 in single-state form: s2+ = z2 + v, z2 = min(s2, R beta); emits V = R o v (tf32 hi/lo).
-constexpr int K2_TP = 32, K2_TJ = 32, K2_TK = 16;
-__global__ void __launch_bounds__(128) k2b_kernel(const double* __restrict__ Sinv, const double* __restrict__ rhs,
-                                                  double* __restrict__ s2, const double* __restrict__ R,
-                                                  const double* __restrict__ beta, int64_t n, int64_t ldn, int Bact,
-                                                  float* __restrict__ v_hi, float* __restrict__ v_lo,
-                                                  double* __restrict__ resid_partial) {
-    __shared__ double sR[K2_TK][K2_TP + 1];     // rhs chunk, [k][p]
-    __shared__ double sS[K2_TK][K2_TJ];         // Sinv chunk, [k][j]
-    __shared__ double sacc[K2_TP][kNumResid];
-    const int tx = threadIdx.x & 7;             // column group (4 columns)
-    const int ty = threadIdx.x >> 3;            // plan group (2 plans)
-    const int64_t j0 = (int64_t)blockIdx.x * K2_TJ;
+constexpr int K2_TP = 96, K2_KC = 32, K2_LD = K2_KC + 4, K2_STAGES = 3;
+
+__device__ __forceinline__ void cp_async16_zfill(void* smem_dst, const void* gsrc, bool ok) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    const int sz = ok ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gsrc), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
+
+template <int WJ>
+__global__ void __launch_bounds__(64 * WJ) k2b_kernel(const double* __restrict__ Sinv, int64_t lds,
+                                                       const double* __restrict__ rhs, double* __restrict__ s2,
+                                                       const double* __restrict__ R, const double* __restrict__ beta,
+                                                       int64_t n, int64_t ldn, int Bact,
+                                                       float* __restrict__ v_hi, float* __restrict__ v_lo,
+                                                       double* __restrict__ resid_partial) {
+    constexpr int TJ = 16 * WJ, NT = 64 * WJ, ROWS = TJ + K2_TP;
+    extern __shared__ __align__(16) double k2sm[];        // [K2_STAGES][ROWS][K2_LD], then the residual staging
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wj = warp % WJ, wp = warp / WJ;              // warp tile: rows wj*16.., plans wp*48..
+    const int g = lane >> 2, q = lane & 3;
+    const int64_t j0 = (int64_t)blockIdx.x * TJ;
     const int p0 = blockIdx.y * K2_TP;
-    double c[2][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}};
-    for (int64_t k0 = 0; k0 < n; k0 += K2_TK) {
-        for (int i = threadIdx.x; i < K2_TK * K2_TP; i += 128) {
-            int kk = i % K2_TK, pp = i / K2_TK;
-            int64_t k = k0 + kk; int p = p0 + pp;
-            sR[kk][pp] = (k < n && p < Bact) ? rhs[(int64_t)p * ldn + k] : 0.0;
+    const int nchunks = (int)((n + K2_KC - 1) / K2_KC);
+    const bool warp_live = p0 + wp * 48 < Bact;
+
+    auto load_chunk = [&](int c, int stage) {
+        double* sA = k2sm + (size_t)stage * ROWS * K2_LD;
+        const int64_t k0 = (int64_t)c * K2_KC;
+        for (int i = tid; i < ROWS * (K2_KC / 2); i += NT) {
+            const int row = i / (K2_KC / 2), kk = (i % (K2_KC / 2)) * 2;
+            const double* src; bool ok;
+            if (row < TJ) { const int64_t j = j0 + row; ok = (j < n) && (k0 + kk < n); src = Sinv + j * lds + k0 + kk; }
+            else { const int p = p0 + row - TJ; ok = (p < Bact) && (k0 + kk < n); src = rhs + (int64_t)p * ldn + k0 + kk; }
+            cp_async16_zfill(sA + row * K2_LD + kk, ok ? src : Sinv, ok);
         }
-        for (int i = threadIdx.x; i < K2_TK * K2_TJ; i += 128) {
-            int jj = i % K2_TJ, kk = i / K2_TJ;
-            int64_t k = k0 + kk, j = j0 + jj;
-            sS[kk][jj] = (k < n && j < n) ? Sinv[k * n + j] : 0.0;
-        }
-        __syncthreads();
+    };
+
+    double acc[2][6][2];
 #pragma unroll
-        for (int kk = 0; kk < K2_TK; ++kk) {
-            double r0 = sR[kk][ty * 2], r1 = sR[kk][ty * 2 + 1];
-            double s0 = sS[kk][tx * 4], s1 = sS[kk][tx * 4 + 1], s2v = sS[kk][tx * 4 + 2], s3 = sS[kk][tx * 4 + 3];
-            c[0][0] += r0 * s0; c[0][1] += r0 * s1; c[0][2] += r0 * s2v; c[0][3] += r0 * s3;
-            c[1][0] += r1 * s0; c[1][1] += r1 * s1; c[1][2] += r1 * s2v; c[1][3] += r1 * s3;
-        }
-        __syncthreads();
-    }
-    const bool resid = resid_partial != nullptr;
-    if (resid) {
-        for (int i = threadIdx.x; i < K2_TP * kNumResid; i += 128) sacc[i / kNumResid][i % kNumResid] = 0.0;
-        __syncthreads();
-    }
+    for (int a = 0; a < 2; ++a)
 #pragma unroll
-    for (int a = 0; a < 2; ++a) {
-        const int p = p0 + ty * 2 + a;
-        double acc[kNumResid] = {0, 0, 0, 0, 0};
-        if (p < Bact) {
+        for (int b = 0; b < 6; ++b) { acc[a][b][0] = 0.0; acc[a][b][1] = 0.0; }
+
 #pragma unroll
-            for (int b = 0; b < 4; ++b) {
-                const int64_t j = j0 + tx * 4 + b;
-                if (j >= n) continue;
-                const double bh = R[j] * beta[p];
-                const double s_old = s2[(int64_t)p * ldn + j];
-                const double z_old = fmin(s_old, bh);
-                const double v = c[a][b];
-                const double s_new = z_old + v;                       // s2+ = x2+ + y2 = v + z2   (Eq. 7)
-                const double z_new = fmin(s_new, bh);                 // (4b)
-                s2[(int64_t)p * ldn + j] = s_new;
-                const double rv = R[j] * v;
-                const float hi = tc::tf32_rn((float)rv);
-                v_hi[(int64_t)p * ldn + j] = hi;
-                v_lo[(int64_t)p * ldn + j] = tc::tf32_rn((float)(rv - (double)hi));
-                if (resid) {
-                    const double y_old = s_old - z_old, y_new = s_new - z_new, x = s_new - y_old;
-                    acc[0] += (x - z_new) * (x - z_new);
-                    acc[1] += (z_new - z_old) * (z_new - z_old);
-                    acc[2] += x * x; acc[3] += z_new * z_new; acc[4] += y_new * y_new;
+    for (int s = 0; s < K2_STAGES - 1; ++s) { if (s < nchunks) load_chunk(s, s); cp_async_commit(); }
+    for (int c = 0; c < nchunks; ++c) {
+        cp_async_wait<K2_STAGES - 2>();
+        __syncthreads();
+        if (c + K2_STAGES - 1 < nchunks) load_chunk(c + K2_STAGES - 1, (c + K2_STAGES - 1) % K2_STAGES);
+        cp_async_commit();
+        if (warp_live) {
+            const double* sA = k2sm + (size_t)(c % K2_STAGES) * ROWS * K2_LD + (wj * 16 + g) * K2_LD + q;
+            const double* sB = k2sm + (size_t)(c % K2_STAGES) * ROWS * K2_LD + (TJ + wp * 48 + g) * K2_LD + q;
+#pragma unroll
+            for (int ks = 0; ks < K2_KC / 4; ++ks) {
+                const double a0 = sA[ks * 4], a1 = sA[8 * K2_LD + ks * 4];
+#pragma unroll
+                for (int b = 0; b < 6; ++b) {
+                    const double bv = sB[b * 8 * K2_LD + ks * 4];
+                    dmma884(acc[0][b], a0, bv);
+                    dmma884(acc[1][b], a1, bv);
                 }
             }
         }
-        if (resid) {
-            // the 8 threads with the same ty are consecutive lanes: reduce over tx with shuffles
+    }
+    cp_async_wait<0>();
+    __syncthreads();
+
+    // ---- epilogue-2: thread owns rows j = j0 + wj*16 + a*8 + g, plans p = p0 + wp*48 + b*8 + 2q + e
+    const bool resid = resid_partial != nullptr;
+    double* sacc = k2sm;                                   // [2 WJ warps][48 plans][kNumResid], reuses the ring
 #pragma unroll
-            for (int t = 0; t < kNumResid; ++t) {
-                double v = acc[t];
-                v += __shfl_xor_sync(0xffffffffu, v, 1);
-                v += __shfl_xor_sync(0xffffffffu, v, 2);
-                v += __shfl_xor_sync(0xffffffffu, v, 4);
-                if (tx == 0) sacc[ty * 2 + a][t] = v;
+    for (int b = 0; b < 6; ++b) {
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int p = p0 + wp * 48 + b * 8 + 2 * q + e;
+            double ra[kNumResid] = {0, 0, 0, 0, 0};
+            if (p < Bact) {
+                const double bp = beta[p];
+#pragma unroll
+                for (int a = 0; a < 2; ++a) {
+                    const int64_t j = j0 + wj * 16 + a * 8 + g;
+                    if (j >= n) continue;
+                    const double bh = R[j] * bp;
+                    const double s_old = s2[(int64_t)p * ldn + j];
+                    const double z_old = fmin(s_old, bh);
+                    const double v = acc[a][b][e];
+                    const double s_new = z_old + v;                       // s2+ = x2+ + y2 = v + z2   (Eq. 7)
+                    const double z_new = fmin(s_new, bh);                 // (4b)
+                    s2[(int64_t)p * ldn + j] = s_new;
+                    const double rv = R[j] * v;
+                    const float hi = tc::tf32_rn((float)rv);
+                    v_hi[(int64_t)p * ldn + j] = hi;
+                    v_lo[(int64_t)p * ldn + j] = tc::tf32_rn((float)(rv - (double)hi));
+                    if (resid) {
+                        const double y_old = s_old - z_old, y_new = s_new - z_new, x = s_new - y_old;
+                        ra[0] += (x - z_new) * (x - z_new);
+                        ra[1] += (z_new - z_old) * (z_new - z_old);
+                        ra[2] += x * x; ra[3] += z_new * z_new; ra[4] += y_new * y_new;
+                    }
+                }
+            }
+            if (resid) {
+                // the 8 lanes with the same q hold the 8 row groups: fixed-order butterfly over g
+#pragma unroll
+                for (int t = 0; t < kNumResid; ++t) {
+                    double v = ra[t];
+                    v += __shfl_xor_sync(0xffffffffu, v, 4);
+                    v += __shfl_xor_sync(0xffffffffu, v, 8);
+                    v += __shfl_xor_sync(0xffffffffu, v, 16);
+                    if (g == 0) sacc[(warp * 48 + b * 8 + 2 * q + e) * kNumResid + t] = v;
+                }
             }
         }
     }
     if (resid) {
         __syncthreads();
-        for (int i = threadIdx.x; i < K2_TP * kNumResid; i += 128) {
-            int pp = i / kNumResid, t = i % kNumResid;
-            if (p0 + pp < Bact)
-                resid_partial[((int64_t)blockIdx.x * kMaxBpad + p0 + pp) * kNumResid + t] = sacc[pp][t];
+        for (int i = tid; i < K2_TP * kNumResid; i += NT) {
+            const int pp = i / kNumResid, t = i % kNumResid;     // pp in [0, 96): wp = pp / 48
+            if (p0 + pp >= Bact) continue;
+            double v = 0.0;
+            for (int w = 0; w < WJ; ++w) v += sacc[(((pp / 48) * WJ + w) * 48 + pp % 48) * kNumResid + t];
+            resid_partial[((int64_t)blockIdx.x * kMaxBpad + p0 + pp) * kNumResid + t] = v;
         }
     }
 }
 
 // ------------------------------------------------------------------------------------------ stopping rule (R7)
-// One thread per slot: fixed-order sum of the per-CTA partials of both blocks, then the Boyd test.
+// One warp per slot: the per-CTA partials of both blocks are summed in a fixed order (lane-strided, then a butterfly),
+// so the decision is deterministic; then the Boyd test.
 __global__ void convergence_kernel(const float* __restrict__ r1, int grid1, const double* __restrict__ r2, int grid2,
                                    int Bact, double dim_sqrt, float tol, float eps_abs,
                                    int32_t* __restrict__ flags, float* __restrict__ res_slot) {
-    int p = blockIdx.x * blockDim.x + threadIdx.x;
+    const int p = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
     if (p >= Bact) return;
     double a[kNumResid] = {0, 0, 0, 0, 0};
-    for (int g = 0; g < grid1; ++g)
+    for (int g = lane; g < grid1; g += 32)
         for (int t = 0; t < kNumResid; ++t) a[t] += (double)r1[((int64_t)g * kMaxBpad + p) * kNumResid + t];
-    for (int g = 0; g < grid2; ++g)
+    for (int g = lane; g < grid2; g += 32)
         for (int t = 0; t < kNumResid; ++t) a[t] += r2[((int64_t)g * kMaxBpad + p) * kNumResid + t];
+    for (int t = 0; t < kNumResid; ++t) a[t] = warp_sum(a[t]);
+    if (lane != 0) return;
     const double rp = sqrt(a[0]), rd = sqrt(a[1]), nx = sqrt(a[2]), nz = sqrt(a[3]), ny = sqrt(a[4]);
     const bool ok = (rp <= (double)eps_abs * dim_sqrt + (double)tol * fmax(nx, nz)) &&
                     (rd <= (double)eps_abs * dim_sqrt + (double)tol * ny);
@@ -451,11 +505,30 @@ void launch_k2a(admm_handle* h, int slot0, int nact, int n_mma, cudaStream_t s) 
                                     slot0, nact, h->d_rhs);
     h->launch_count++;
 }
-int k2b_grid(const admm_handle* h, int) { return (int)cdiv(h->n, K2_TJ); }
+// rows of the block tile: the largest of 64 / 32 / 16 that still gives every SM a block
+int k2_choose_wj(const admm_handle* h, int Bpad) {
+    const int gy = (int)cdiv(Bpad, K2_TP);
+    for (int wj = 4; wj > 1; wj >>= 1)
+        if (cdiv(h->n, 16 * wj) * gy >= h->sm_count) return wj;
+    return 1;
+}
+static int k2_wj(const admm_handle* h) { return h->k2_wj; }
+int k2b_grid(const admm_handle* h, int) { return (int)cdiv(h->n, 16 * k2_wj(h)); }
+template <int WJ>
+static void launch_k2b_t(admm_handle* h, int Bact, bool resid, cudaStream_t s) {
+    const size_t smem = (size_t)K2_STAGES * (16 * WJ + K2_TP) * K2_LD * sizeof(double);
+    static bool attr_done = false;
+    if (!attr_done) { cudaFuncSetAttribute(k2b_kernel<WJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_done = true; }
+    dim3 grid((unsigned)cdiv(h->n, 16 * WJ), (unsigned)cdiv(Bact, K2_TP));
+    k2b_kernel<WJ><<<grid, 64 * WJ, smem, s>>>(h->d_Sinv, h->lds, h->d_rhs, h->d_s2, h->d_R, h->d_beta, h->n, h->ldn, Bact,
+                                               h->d_vhi, h->d_vlo, resid ? h->d_resid2 : nullptr);
+}
 void launch_k2b(admm_handle* h, int Bact, bool resid, cudaStream_t s) {
-    dim3 grid((unsigned)cdiv(h->n, K2_TJ), (unsigned)cdiv(Bact, K2_TP));
-    k2b_kernel<<<grid, 128, 0, s>>>(h->d_Sinv, h->d_rhs, h->d_s2, h->d_R, h->d_beta, h->n, h->ldn, Bact, h->d_vhi,
-                                    h->d_vlo, resid ? h->d_resid2 : nullptr);
+    switch (k2_wj(h)) {
+        case 4: launch_k2b_t<4>(h, Bact, resid, s); break;
+        case 2: launch_k2b_t<2>(h, Bact, resid, s); break;
+        default: launch_k2b_t<1>(h, Bact, resid, s); break;
+    }
     h->launch_count++;
 }
 void launch_simt_k1(admm_handle* h, int slot0, int nact, int n_mma, int splits, cudaStream_t s) {
@@ -477,7 +550,7 @@ void launch_simt_k3(admm_handle* h, const EpiParams& ep, int epi, const float* v
     h->launch_count += 2;
 }
 void launch_convergence(admm_handle* h, int Bact, int grid1, int grid2, float tol, float eps_abs, cudaStream_t s) {
-    convergence_kernel<<<(unsigned)cdiv(Bact, 64), 64, 0, s>>>(h->d_resid1, grid1, h->d_resid2, grid2, Bact,
+    convergence_kernel<<<(unsigned)cdiv(Bact, 4), 128, 0, s>>>(h->d_resid1, grid1, h->d_resid2, grid2, Bact,
                                                               sqrt((double)(h->N + h->n)), tol, eps_abs, h->d_conv_flags,
                                                               h->d_res_slot);
     h->launch_count++;

@@ -65,7 +65,9 @@ def test_contractions_match_fp64_matmul(b, shape):
 
 def test_accumulation_is_unbiased(b):
     """tcgen05.mma accumulates with round-toward-zero; the drained fp32 path must not show that bias
-    (all-positive operands, K = 4800: undrained it is -3e-5 of the sum)."""
+    (all-positive operands, K = 4800: undrained it is -3e-5 of the sum).
+    What is left is the truncation inside one drain interval (4 MMAs of one 32-element k-block, each cut
+    ~0.45 ulp of the CHUNK sum): about -1.5e-7 of the total whatever K is, i.e. ~1 ulp of fp32."""
     from workloads import make_workload
     w = make_workload(0, n_target=300, n_lowdose=500, n_iso=200)
     small = np.abs(np.random.default_rng(2).standard_normal((16, w.n))).astype(np.float32)
@@ -74,7 +76,7 @@ def test_accumulation_is_unbiased(b):
     h.close()
     exact = small.astype(np.float64) @ w.phi.astype(np.float64).T
     rel = (got - exact) / exact
-    assert abs(np.mean(rel)) < 1e-7 and np.max(np.abs(rel)) < 1e-6
+    assert abs(np.mean(rel)) < 3e-7 and np.max(np.abs(rel)) < 1e-6
 
 
 # ------------------------------------------------------------------------------------------ fixed-K iterate parity
@@ -104,10 +106,12 @@ def test_fixed_k_parity_row_masks_multitarget(b):
 
 
 def test_fixed_k_parity_more_than_one_pass_of_plans(b):
-    """B = 144 > 96: the fp32 path runs the contractions in two passes over the plans."""
+    """B = 144 > 96: the fp32 path runs the contractions in two passes over the plans.  K = 50 as north_star fixes
+    it (at K = 30 the (0,0) plan is mid-transient with ||z|| = 6e-3 ||y||: z = clip(s) then carries the fp32
+    rounding noise of s, ~1e-6 ||s||, which is 2e-4 of ||z|| -- DESIGN.md section 7 "cancellation")."""
     from workloads import default_rho, make_workload
     w = make_workload(0, n_target=600, n_lowdose=1200, n_iso=4, grid=12)
-    ez, ey, et, _, _, _ = _parity(b, w, default_rho(w.beta), 30)
+    ez, ey, et, _, _, _ = _parity(b, w, default_rho(w.beta), 50)
     assert ez.max() < TOL_FP32 and ey.max() < TOL_FP32 and et.max() < TOL_FP32
 
 
@@ -233,7 +237,9 @@ def test_single_plan_and_degenerate_weights(b):
     """B = 1; alpha = beta = 0 (optimum 0, every iterate of z stays 0); beta large (t* = 0, OPT = 1)."""
     from workloads import make_workload
     w = make_workload(0, n_target=300, n_lowdose=500, n_iso=4)
-    h = b.admm_setup(w.phi, w.point_class, w.classes)
+    # eps_abs = 1e-5: for this plan x, z -> 0 while ||y|| = 26, so the relative part of the rule vanishes and the
+    # primal residual sits on the fp32 rounding floor of s (~1.5e-6 ||y|| = 3e-5 = the default 1e-6 sqrt(N+n) exactly)
+    h = b.admm_setup(w.phi, w.point_class, w.classes, eps_abs=1e-5)
     out = b.admm_solve_batch(h, np.array([[1.0, 0.0, 0.0]]), np.array([1e-3]), tol=1e-4, max_iter=500)
     assert out["obj"][0] < 1e-6 and out["iters"][0] <= 100
     bound = w.phi[w.point_class == 0].astype(np.float64).mean(axis=0).max()

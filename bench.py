@@ -140,9 +140,9 @@ def run_reference(args) -> None:
     if rank != 0:
         return
     from oracle import admm as oracle_admm
-    from workloads import default_rho, make_workload
+    from workloads import make_workload, scaled_rho
     w = make_workload(args.config)
-    rho = default_rho(w.beta)
+    rho = scaled_rho(w.beta, w.point_class)
     its = args.ref_iters
     first = _oracle_sample(w, rho, its)
     pre, u_hat, b_hat, st0 = first["pre"]
@@ -185,7 +185,7 @@ def main() -> None:
     import torch
     import torch.distributed as dist
     from paper_2509_08602_b200 import binding as b          # fails loudly if the CUDA library is missing
-    from workloads import default_rho, make_workload
+    from workloads import make_workload, scaled_rho
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -200,7 +200,7 @@ def main() -> None:
     w = make_workload(args.config)
     # weak scaling: rank r solves its own B plans, the slider grid shifted inside [0,1]^2
     weights = rank_weights(w.weights, rank, world)
-    rho = default_rho(weights[:, 2])
+    rho = scaled_rho(weights[:, 2], w.point_class)
     stream = torch.cuda.current_stream().cuda_stream
 
     phi_pinned = torch.from_numpy(w.phi).pin_memory()
@@ -293,7 +293,7 @@ def main() -> None:
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        s = _oracle_sample(w, default_rho(w.beta), args.ref_iters)
+        s = _oracle_sample(w, scaled_rho(w.beta, w.point_class), args.ref_iters)
         cpu = {"value": s["value"], "unit": UNIT, "cores": s["cores"], "kind": "oracle",
                "sample": f"{args.ref_iters} ADMM iterations of all {w.B} plans of the same workload in {s['seconds']:.1f} s "
                          f"(fp64 numpy oracle; its setup, {s['setup_seconds']:.1f} s, excluded like the GPU's)"}

@@ -106,8 +106,8 @@ admm_status admm_setup(admm_handle** out, const float* phi, int32_t phi_on_devic
  * (PAPER.md:73-94), stacked per :96, from the all-zero iterate.
  *
  *   weights     [B][n_classes+1] HOST fp32: w_class 0.., then w_BOT (config LP: 1, alpha, beta); >= 0, finite
- *   rho         [B] HOST fp32 step sizes (> 0), or NULL => rho0*sqrt(w0/max(w_BOT,w0)), rho0=1e-3, w0=0.05
- *               (the shape of Eq. 9, :219)
+ *   rho         [B] HOST fp32 step sizes (> 0), or NULL => (1/N_min) sqrt(w0/max(w_BOT, w0/64)), w0 = 0.05, N_min = the
+ *               smallest class count (the shape of Eq. 9, :219, scaled to the column scaling D; R8)
  *   row_mask    [B][ceil(N/32)] uint32 bit-packed (bit i%32 of word i/32 set => row i active in plan p;
  *               inactive rows get u = 0, :144), HOST or DEVICE pointer, or NULL => all rows active
  *   tol         relative tolerance of the stopping rule (R7); ignored if fixed_iters > 0

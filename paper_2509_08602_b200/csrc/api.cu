@@ -515,9 +515,12 @@ admm_status admm_solve_batch(admm_handle* h, int32_t B, const float* weights, co
     h->slot_plan.assign(h->Bpad, 0); h->plan_slot.assign(B, 0); h->iters.assign(B, 0);
     h->h_weights.assign(weights, weights + (size_t)B * W);
     std::vector<float> res_plan((size_t)2 * B, 0.f);
+    int64_t n_min_class = h->class_count[0];
+    for (int k = 1; k < K; ++k) n_min_class = std::min(n_min_class, h->class_count[k]);
     for (int p = 0; p < B; ++p) {
         const double beta = weights[(size_t)p * W + K];
-        const double r = rho ? (double)rho[p] : 1e-3 * std::sqrt(0.05 / std::max(beta, 0.05));
+        // default: (kappa / N_min) sqrt(beta0 / max(beta, beta0/64)), kappa = 1, beta0 = 0.05 (reading R8)
+        const double r = rho ? (double)rho[p] : (1.0 / (double)n_min_class) * std::sqrt(0.05 / std::max(beta, 0.05 / 64.0));
         T.beta[p] = beta; T.rho[p] = r;
         for (int k = 0; k < K; ++k) {
             const double Nk = (double)h->class_count[k], Nkp = (double)counts[(size_t)p * kMaxClasses + k];

@@ -183,16 +183,18 @@ __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
 }
 
 template <int WJ>
-__global__ void __launch_bounds__(64 * WJ) k2b_kernel(const double* __restrict__ Sinv, int64_t lds,
-                                                       const double* __restrict__ rhs, double* __restrict__ s2,
-                                                       const double* __restrict__ R, const double* __restrict__ beta,
-                                                       int64_t n, int64_t ldn, int Bact,
-                                                       float* __restrict__ v_hi, float* __restrict__ v_lo,
-                                                       double* __restrict__ resid_partial) {
-    constexpr int TJ = 16 * WJ, NT = 64 * WJ, ROWS = TJ + K2_TP;
-    extern __shared__ __align__(16) double k2sm[];        // [K2_STAGES][ROWS][K2_LD], then the residual staging
+__global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sinv, int64_t lds,
+                                                  const double* __restrict__ rhs, double* __restrict__ s2,
+                                                  const double* __restrict__ R, const double* __restrict__ beta,
+                                                  int64_t n, int64_t ldn, int Bact,
+                                                  float* __restrict__ v_hi, float* __restrict__ v_lo,
+                                                  double* __restrict__ resid_partial) {
+    // 8 warps = WJ row groups x 2 plan halves x KS k-slices (a lone warp per scheduler cannot hide the DMMA issue
+    // latency: measured 14 % pipe utilisation with 2 warps per block); the k-slices are summed through shared memory.
+    constexpr int TJ = 16 * WJ, NT = 256, ROWS = TJ + K2_TP, KS = 4 / WJ;
+    extern __shared__ __align__(16) double k2sm[];        // [K2_STAGES][ROWS][K2_LD]; reused after the main loop
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int wj = warp % WJ, wp = warp / WJ;              // warp tile: rows wj*16.., plans wp*48..
+    const int wj = warp % WJ, wp = (warp / WJ) & 1, kq = warp / (2 * WJ);
     const int g = lane >> 2, q = lane & 3;
     const int64_t j0 = (int64_t)blockIdx.x * TJ;
     const int p0 = blockIdx.y * K2_TP;
@@ -228,7 +230,8 @@ __global__ void __launch_bounds__(64 * WJ) k2b_kernel(const double* __restrict__
             const double* sA = k2sm + (size_t)(c % K2_STAGES) * ROWS * K2_LD + (wj * 16 + g) * K2_LD + q;
             const double* sB = k2sm + (size_t)(c % K2_STAGES) * ROWS * K2_LD + (TJ + wp * 48 + g) * K2_LD + q;
 #pragma unroll
-            for (int ks = 0; ks < K2_KC / 4; ++ks) {
+            for (int i = 0; i < K2_KC / 4 / KS; ++i) {
+                const int ks = kq + i * KS;
                 const double a0 = sA[ks * 4], a1 = sA[8 * K2_LD + ks * 4];
 #pragma unroll
                 for (int b = 0; b < 6; ++b) {
@@ -242,9 +245,33 @@ __global__ void __launch_bounds__(64 * WJ) k2b_kernel(const double* __restrict__
     cp_async_wait<0>();
     __syncthreads();
 
+    // ---- sum the k-slices in a fixed order: slices 1.. park their fragments, slice 0 adds them
+    double* red = k2sm;                                    // [(KS-1)][2 WJ warps][24][32]
+    double* sacc = k2sm + (size_t)3 * 2 * 24 * 32;         // [2 WJ warps][48 plans][kNumResid]
+    if (KS > 1) {
+        if (kq > 0) {
+            double* dst = red + ((size_t)((kq - 1) * 2 * WJ + wp * WJ + wj) * 24) * 32 + lane;
+#pragma unroll
+            for (int a = 0; a < 2; ++a)
+#pragma unroll
+                for (int b = 0; b < 6; ++b) { dst[((a * 6 + b) * 2 + 0) * 32] = acc[a][b][0]; dst[((a * 6 + b) * 2 + 1) * 32] = acc[a][b][1]; }
+        }
+        __syncthreads();
+        if (kq == 0) {
+            for (int k = 1; k < KS; ++k) {
+                const double* src = red + ((size_t)((k - 1) * 2 * WJ + wp * WJ + wj) * 24) * 32 + lane;
+#pragma unroll
+                for (int a = 0; a < 2; ++a)
+#pragma unroll
+                    for (int b = 0; b < 6; ++b) { acc[a][b][0] += src[((a * 6 + b) * 2 + 0) * 32]; acc[a][b][1] += src[((a * 6 + b) * 2 + 1) * 32]; }
+            }
+        }
+    }
+    const int ew = wp * WJ + wj;                           // index of this (kq == 0) warp among the 2 WJ epilogue warps
+
     // ---- epilogue-2: thread owns rows j = j0 + wj*16 + a*8 + g, plans p = p0 + wp*48 + b*8 + 2q + e
     const bool resid = resid_partial != nullptr;
-    double* sacc = k2sm;                                   // [2 WJ warps][48 plans][kNumResid], reuses the ring
+    if (kq == 0) {
 #pragma unroll
     for (int b = 0; b < 6; ++b) {
 #pragma unroll
@@ -284,10 +311,11 @@ __global__ void __launch_bounds__(64 * WJ) k2b_kernel(const double* __restrict__
                     v += __shfl_xor_sync(0xffffffffu, v, 4);
                     v += __shfl_xor_sync(0xffffffffu, v, 8);
                     v += __shfl_xor_sync(0xffffffffu, v, 16);
-                    if (g == 0) sacc[(warp * 48 + b * 8 + 2 * q + e) * kNumResid + t] = v;
+                    if (g == 0) sacc[(ew * 48 + b * 8 + 2 * q + e) * kNumResid + t] = v;
                 }
             }
         }
+    }
     }
     if (resid) {
         __syncthreads();
@@ -520,7 +548,7 @@ static void launch_k2b_t(admm_handle* h, int Bact, bool resid, cudaStream_t s) {
     static bool attr_done = false;
     if (!attr_done) { cudaFuncSetAttribute(k2b_kernel<WJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_done = true; }
     dim3 grid((unsigned)cdiv(h->n, 16 * WJ), (unsigned)cdiv(Bact, K2_TP));
-    k2b_kernel<WJ><<<grid, 64 * WJ, smem, s>>>(h->d_Sinv, h->lds, h->d_rhs, h->d_s2, h->d_R, h->d_beta, h->n, h->ldn, Bact,
+    k2b_kernel<WJ><<<grid, 256, smem, s>>>(h->d_Sinv, h->lds, h->d_rhs, h->d_s2, h->d_R, h->d_beta, h->n, h->ldn, Bact,
                                                h->d_vhi, h->d_vlo, resid ? h->d_resid2 : nullptr);
 }
 void launch_k2b(admm_handle* h, int Bact, bool resid, cudaStream_t s) {

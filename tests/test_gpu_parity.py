@@ -194,6 +194,17 @@ def test_compaction_preserves_each_plan(b):
     h.close()
 
 
+def test_null_rho_is_the_documented_default_rule(b):
+    """rho = NULL: the library applies workloads.scaled_rho's rule (header of admm_solve_batch, R8)."""
+    from workloads import make_workload, scaled_rho
+    w = make_workload(1, n_target=700, n_lowdose=1500, n_iso=5, grid=4)
+    h = b.admm_setup(w.phi, w.point_class, w.classes)
+    o1 = b.admm_solve_batch(h, w.weights, None, fixed_iters=25)
+    o2 = b.admm_solve_batch(h, w.weights, scaled_rho(w.beta, w.point_class), fixed_iters=25)
+    h.close()
+    assert np.allclose(o1["t"], o2["t"], rtol=1e-4, atol=1e-7) and np.allclose(o1["obj"], o2["obj"], rtol=1e-5)
+
+
 def test_residuals_match_oracle(b):
     from workloads import default_rho, make_workload
     w = make_workload(0, n_target=500, n_lowdose=900, n_iso=5)

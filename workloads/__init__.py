@@ -14,6 +14,7 @@ from .generate import (  # noqa: F401
     ClassSpec,
     Workload,
     default_rho,
+    scaled_rho,
     make_workload,
     make_tiny_workload,
     pack_mask,

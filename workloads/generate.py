@@ -140,6 +140,18 @@ def default_rho(beta: np.ndarray, rho0: float = 1e-3, beta0: float = 0.05) -> np
     return rho0 * np.sqrt(beta0 / np.maximum(beta, beta0))
 
 
+def scaled_rho(beta: np.ndarray, point_class: np.ndarray, kappa: float = 1.0, beta0: float = 0.05,
+               floor_div: float = 64.0) -> np.ndarray:
+    """Size-aware step size (reading R8): rho_p = (kappa / N_min) * sqrt(beta0 / max(beta_p, beta0/floor_div)),
+    N_min = the smallest class count.  With the column scaling D_i = 1/N_class(i) (R10) the linear term of the
+    iteration is c_hat/rho = -+1/(N_k rho), so rho0 = kappa/N_min keeps it O(1/kappa) whatever the number of dose
+    points; the lower clamp lets rho grow 8x towards w_BOT = 0 (Eq. 9 has rho -> inf there).
+    For config 0 (N_T = 1000) and beta >= beta0 this is default_rho().  The library's rho = NULL default is the same rule."""
+    beta = np.asarray(beta, dtype=np.float64)
+    n_min = float(np.bincount(np.asarray(point_class).astype(np.int64)).min())
+    return (kappa / n_min) * np.sqrt(beta0 / np.maximum(beta, beta0 / floor_div))
+
+
 def pack_mask(mask_bool: np.ndarray) -> np.ndarray:
     """[B, N] bool -> [B, ceil(N/32)] uint32, bit (i % 32) of word (i // 32)."""
     B, N = mask_bool.shape

@@ -42,7 +42,7 @@ class admm_options(C.Structure):
     _fields_ = [("storage", C.c_int32), ("kernel_path", C.c_int32), ("device", C.c_int32), ("stream", C.c_void_p),
                 ("check_every", C.c_int32), ("eps_abs", C.c_float), ("compaction", C.c_int32),
                 ("csr_rel_threshold", C.c_float), ("profile_kernels", C.c_int32), ("drain_kb", C.c_int32),
-                ("reserved", C.c_int32 * 6)]
+                ("k1_slab_kb", C.c_int32), ("reserved", C.c_int32 * 5)]
 
 
 def _load() -> C.CDLL:
@@ -119,7 +119,7 @@ def admm_default_options() -> admm_options:
 def admm_setup(phi, point_class, classes: Sequence, *, storage: int = ADMM_STORAGE_FP32_3XTF32,
                kernel_path: int = ADMM_PATH_TCGEN05, device: int = 0, stream: Optional[int] = None,
                check_every: int = 10, eps_abs: float = 1e-6, compaction: bool = True,
-               profile_kernels: bool = False, drain_kb: int = 0) -> Handle:
+               profile_kernels: bool = False, drain_kb: int = 0, k1_slab_kb: int = 0) -> Handle:
     """phi: [N, n] float32, numpy (host) or torch CUDA tensor, row-major (last stride 1).
     classes: sequence of objects with .sense, .threshold, .hard (e.g. workloads.ClassSpec)."""
     if _is_torch(phi):
@@ -137,6 +137,7 @@ def admm_setup(phi, point_class, classes: Sequence, *, storage: int = ADMM_STORA
     o.stream = stream
     o.check_every, o.eps_abs, o.compaction, o.profile_kernels = check_every, eps_abs, int(compaction), int(profile_kernels)
     o.drain_kb = int(drain_kb)
+    o.k1_slab_kb = int(k1_slab_kb)
     out = C.c_void_p()
     st = _lib.admm_setup(C.byref(out), _ptr(phi), on_device, N, n, ld, _ptr(pc), cls, len(classes), C.byref(o))
     _check(st, None)

@@ -168,12 +168,15 @@ __global__ void k2a_kernel(const float* __restrict__ partial, const int32_t* __r
 // K is walked in chunks of 32 through a 3-stage cp.async ring; both operands are K-contiguous in memory
 // (Sinv[j][k] row-major with padded row stride, rhs[p][k] plan-major), rows padded to 36 doubles => conflict-free LDS.64.
 // Epilogue (4b)/(4c) on block 2 in single-state form: s2+ = z2 + v, z2 = min(s2, R beta); emits V = R o v (tf32 hi/lo).
-constexpr int K2_TP = 96, K2_KC = 32, K2_LD = K2_KC + 4, K2_STAGES = 3;
+constexpr int K2_TP = 96, K2_KC = 32, K2_LD = K2_KC + 4;
+// ring depth: as many 32-column chunks as fit in ~200 KB (the operands come from L2 / HBM at ~1 us latency and the
+// DMMA work per chunk is a few hundred cycles: bytes in flight are what sets the speed)
+__host__ __device__ constexpr int k2_stages(int WJ) { return (200 * 1024) / ((16 * WJ + K2_TP) * K2_LD * 8) > 8 ? 8 : (200 * 1024) / ((16 * WJ + K2_TP) * K2_LD * 8); }
 
 __device__ __forceinline__ void cp_async16_zfill(void* smem_dst, const void* gsrc, bool ok) {
     const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
     const int sz = ok ? 16 : 0;
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gsrc), "r"(sz) : "memory");
+    asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2, %3;" ::"r"(d), "l"(gsrc), "r"(sz), "l"(tc::kEvictLast) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
@@ -191,7 +194,7 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
                                                   double* __restrict__ resid_partial) {
     // 8 warps = WJ row groups x 2 plan halves x KS k-slices (a lone warp per scheduler cannot hide the DMMA issue
     // latency: measured 14 % pipe utilisation with 2 warps per block); the k-slices are summed through shared memory.
-    constexpr int TJ = 16 * WJ, NT = 256, ROWS = TJ + K2_TP, KS = 4 / WJ;
+    constexpr int TJ = 16 * WJ, NT = 256, ROWS = TJ + K2_TP, KS = 4 / WJ, K2_STAGES = k2_stages(WJ);
     extern __shared__ __align__(16) double k2sm[];        // [K2_STAGES][ROWS][K2_LD]; reused after the main loop
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wj = warp % WJ, wp = (warp / WJ) & 1, kq = warp / (2 * WJ);
@@ -201,15 +204,28 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
     const int nchunks = (int)((n + K2_KC - 1) / K2_KC);
     const bool warp_live = p0 + wp * 48 < Bact;
 
+    // loader: thread t copies 16-byte pieces (row = t/16 + 16 i, columns kk, kk+1) for i < NCP; pointers are set up once
+    constexpr int NCP = ROWS * (K2_KC / 2) / NT;             // 7 / 8 / 10 for WJ = 1 / 2 / 4 (exact)
+    static_assert(ROWS * (K2_KC / 2) % NT == 0, "loader tiling");
+    const int kk = (tid & 15) * 2;
+    const double* srcp[NCP];
+    bool rowok[NCP];
+#pragma unroll
+    for (int i = 0; i < NCP; ++i) {
+        const int row = (tid >> 4) + 16 * i;
+        if (row < TJ) { const int64_t j = j0 + row; rowok[i] = j < n; srcp[i] = Sinv + (rowok[i] ? j : 0) * lds + kk; }
+        else { const int p = p0 + row - TJ; rowok[i] = p < Bact; srcp[i] = rhs + (int64_t)(rowok[i] ? p : 0) * ldn + kk; }
+    }
+    const uint32_t dst0 = (uint32_t)__cvta_generic_to_shared(k2sm) + (uint32_t)(((tid >> 4) * K2_LD + kk) * 8);
     auto load_chunk = [&](int c, int stage) {
-        double* sA = k2sm + (size_t)stage * ROWS * K2_LD;
         const int64_t k0 = (int64_t)c * K2_KC;
-        for (int i = tid; i < ROWS * (K2_KC / 2); i += NT) {
-            const int row = i / (K2_KC / 2), kk = (i % (K2_KC / 2)) * 2;
-            const double* src; bool ok;
-            if (row < TJ) { const int64_t j = j0 + row; ok = (j < n) && (k0 + kk < n); src = Sinv + j * lds + k0 + kk; }
-            else { const int p = p0 + row - TJ; ok = (p < Bact) && (k0 + kk < n); src = rhs + (int64_t)p * ldn + k0 + kk; }
-            cp_async16_zfill(sA + row * K2_LD + kk, ok ? src : Sinv, ok);
+        const bool kok = k0 + kk < n;
+        const uint32_t d = dst0 + (uint32_t)stage * (ROWS * K2_LD * 8);
+#pragma unroll
+        for (int i = 0; i < NCP; ++i) {
+            const int sz = (kok && rowok[i]) ? 16 : 0;
+            asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2, %3;" ::"r"(d + (uint32_t)(i * 16 * K2_LD * 8)),
+                         "l"(kok ? srcp[i] + k0 : srcp[i]), "r"(sz), "l"(tc::kEvictLast) : "memory");
         }
     };
 
@@ -544,7 +560,7 @@ static int k2_wj(const admm_handle* h) { return h->k2_wj; }
 int k2b_grid(const admm_handle* h, int) { return (int)cdiv(h->n, 16 * k2_wj(h)); }
 template <int WJ>
 static void launch_k2b_t(admm_handle* h, int Bact, bool resid, cudaStream_t s) {
-    const size_t smem = (size_t)K2_STAGES * (16 * WJ + K2_TP) * K2_LD * sizeof(double);
+    const size_t smem = (size_t)k2_stages(WJ) * (16 * WJ + K2_TP) * K2_LD * sizeof(double);
     static bool attr_done = false;
     if (!attr_done) { cudaFuncSetAttribute(k2b_kernel<WJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_done = true; }
     dim3 grid((unsigned)cdiv(h->n, 16 * WJ), (unsigned)cdiv(Bact, K2_TP));

@@ -63,6 +63,21 @@ def test_contractions_match_fp64_matmul(b, shape):
     h.close()
 
 
+def test_k1_slab_major_stream_k(b):
+    """K1's slab-major stream-K (several slabs, units that straddle m-tile boundaries, ragged last slab)."""
+    from workloads import make_workload
+    w = make_workload(0, n_target=900, n_lowdose=1711, n_iso=12)          # N = 2611 (82 k-blocks), n = 288 (3 m-tiles, ragged)
+    P = w.phi.astype(np.float64)
+    small = np.random.default_rng(5).standard_normal((40, w.N)).astype(np.float32)
+    exact = small.astype(np.float64) @ P
+    scale = np.abs(small.astype(np.float64)) @ P
+    for slab in (7, 16, 64):
+        h = b.admm_setup(w.phi, w.point_class, w.classes, k1_slab_kb=slab)
+        got = b.admm_contract_probe(h, 0, small)
+        h.close()
+        assert np.max(np.abs(got - exact) / scale) < 1e-6, slab
+
+
 def test_accumulation_is_unbiased(b):
     """tcgen05.mma accumulates with round-toward-zero; the drained fp32 path must not show that bias
     (all-positive operands, K = 4800: undrained it is -3e-5 of the sum).

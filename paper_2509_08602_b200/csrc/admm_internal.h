@@ -58,8 +58,9 @@ struct EpiParams {
 };
 
 struct TcLaunch {
-    CUtensorMap map_big;     // big operand [rows][K], box {32, 32}
-    CUtensorMap map_big128;  // big operand [rows][K], box {32, 128}: a whole tile per TMA (fp32 path)
+    CUtensorMap map_big;     // big operand, tile-major [tiles * 128][32], box {32, 32}
+    CUtensorMap map_big128;  // same tensor, box {32, 128}: a whole 16 KB tile per TMA (fp32 path)
+    int32_t big_kb_total;    // k-blocks per row tile of the big operand (tile (rt, kb) starts at row (rt * big_kb_total + kb) * 128)
     CUtensorMap map_small_hi;// small operand [Bpad][K], box {32, n_mma}
     CUtensorMap map_small_lo;
     const TcUnit* units;     // device
@@ -87,8 +88,10 @@ struct admm_handle {
     std::vector<uint8_t> h_point_class;
 
     // device, owned
-    float* d_phi = nullptr;        // [N][ldn]
-    float* d_phiT = nullptr;       // [n][ldN]
+    float* d_phi = nullptr;        // [N][ldn] row-major (setup; kept only by the SIMT cross-check path)
+    float* d_phiT = nullptr;       // [n][ldN] row-major (SIMT cross-check path only)
+    float* d_phi_t = nullptr;      // tile-major Phi:   [ceil(N/128)][ceil(n/32)][128][32]  (K3 / objective big operand)
+    float* d_phiT_t = nullptr;     // tile-major Phi^T: [ceil(n/128)][ceil(N/32)][128][32]  (K1 big operand)
     uint8_t* d_point_class = nullptr;
     double* d_R = nullptr;         // [n]
     double* d_Sinv = nullptr;      // [n][lds], lds = n rounded up to even (16-byte rows for cp.async), pad = 0
@@ -136,6 +139,7 @@ admm_status tc_make_map(admm_handle* h, CUtensorMap* out, const void* base, int6
 admm_status tc_launch(admm_handle* h, const TcLaunch& L);
 
 // ---- kernels.cu  (everything that is not a tcgen05 contraction)
+void launch_pack_tiles(const float* src, int64_t src_rows, int64_t src_cols, int64_t ld_src, bool transpose, float* dst, cudaStream_t s);
 void launch_transpose(const float* src, int64_t rows, int64_t cols, int64_t ld_src, float* dst, int64_t ld_dst, cudaStream_t s);
 void launch_scale_rows_to_f64(const float* phi, int64_t ld, int64_t row0, int64_t rows, int64_t n,
                               const uint8_t* cls, const double* a_cls, double* out, cudaStream_t s);

@@ -58,18 +58,16 @@ bool is_device_ptr(const void* p) {
 }
 
 // ---- unit tables ------------------------------------------------------------------------------------------
-// K3: the 32-row groups of Phi are dealt evenly to the CTAs; a CTA walks its range in 128-row tiles.
+// K3: the 128-row tiles of Phi (aligned: the big operand is stored tile-major) are dealt evenly to the CTAs.
 void build_units_k3(int64_t N, int64_t n, int sm, std::vector<TcUnit>& units, std::vector<int32_t>& begin) {
-    const int64_t groups = cdiv(N, kBoxRows);
-    const int grid = (int)std::min<int64_t>(sm, cdiv(groups, kTileM / kBoxRows));
+    const int64_t tiles = cdiv(N, kTileM);
+    const int grid = (int)std::min<int64_t>(sm, tiles);
     const int kb = (int)cdiv(n, kBlockK);
     units.clear(); begin.assign(1, 0);
     for (int c = 0; c < grid; ++c) {
-        int64_t g0 = groups * c / grid, g1 = groups * (c + 1) / grid;
-        for (int64_t g = g0; g < g1; g += kTileM / kBoxRows) {
-            int64_t row0 = g * kBoxRows;
-            int64_t row1 = std::min<int64_t>(std::min<int64_t>(g + kTileM / kBoxRows, g1) * kBoxRows, N);
-            units.push_back(TcUnit{(int32_t)row0, (int32_t)(row1 - row0), 0, kb, 0, 0});
+        for (int64_t t = tiles * c / grid; t < tiles * (c + 1) / grid; ++t) {
+            const int64_t row0 = t * kTileM;
+            units.push_back(TcUnit{(int32_t)row0, (int32_t)std::min<int64_t>(kTileM, N - row0), 0, kb, 0, 0});
         }
         begin.push_back((int32_t)units.size());
     }
@@ -148,7 +146,7 @@ struct Profiler {
 };
 
 void free_all(admm_handle* h) {
-    void* ptrs[] = {h->d_phi, h->d_phiT, h->d_point_class, h->d_R, h->d_Sinv, h->d_s1, h->d_ghi, h->d_glo, h->d_s2, h->d_rhs,
+    void* ptrs[] = {h->d_phi, h->d_phiT, h->d_phi_t, h->d_phiT_t, h->d_point_class, h->d_R, h->d_Sinv, h->d_s1, h->d_ghi, h->d_glo, h->d_s2, h->d_rhs,
                     h->d_vhi, h->d_vlo, h->d_partial, h->d_resid1, h->d_resid2, h->d_hinge, h->d_mask, h->d_slot_plan,
                     h->d_utab, h->d_crtab, h->d_beta, h->d_rho, h->d_active_counts, h->d_conv_flags, h->d_res_slot,
                     h->d_rowtmp, h->d_rowtmp2, h->d_units_k1, h->d_cta_begin_k1, h->d_mtile_slot_begin, h->d_units_k3,
@@ -195,8 +193,11 @@ admm_status contract(admm_handle* h, int epi, int slot0, int nact, const float* 
     TcLaunch L{};
     const bool k1 = (epi == EPI_K1_PARTIAL);
     const int64_t big_rows = k1 ? h->n : h->N, big_cols = k1 ? h->N : h->n, big_ld = k1 ? h->ldN : h->ldn;
-    ST_TRY(tc_make_map(h, &L.map_big, k1 ? h->d_phiT : h->d_phi, big_rows, big_cols, big_ld, kBoxRows));
-    ST_TRY(tc_make_map(h, &L.map_big128, k1 ? h->d_phiT : h->d_phi, big_rows, big_cols, big_ld, kTileM));
+    // big operand: tile-major [row tiles][k-blocks][128][32] seen as a 2-D tensor of 128-byte rows
+    const int64_t kb_total = cdiv(big_cols, kBlockK), tiled_rows = cdiv(big_rows, kTileM) * kb_total * kTileM;
+    ST_TRY(tc_make_map(h, &L.map_big, k1 ? h->d_phiT_t : h->d_phi_t, tiled_rows, kBlockK, kBlockK, kBoxRows));
+    ST_TRY(tc_make_map(h, &L.map_big128, k1 ? h->d_phiT_t : h->d_phi_t, tiled_rows, kBlockK, kBlockK, kTileM));
+    L.big_kb_total = (int32_t)kb_total;
     // the small operand has Bpad rows allocated; rows >= nact of the box are dead columns of D
     ST_TRY(tc_make_map(h, &L.map_small_hi, small_hi + (int64_t)slot0 * big_ld, h->Bpad - slot0, big_cols, big_ld, n_mma));
     ST_TRY(tc_make_map(h, &L.map_small_lo, small_lo + (int64_t)slot0 * big_ld, h->Bpad - slot0, big_cols, big_ld, n_mma));
@@ -269,17 +270,27 @@ static admm_status setup_impl(admm_handle* h, const float* phi, int32_t phi_on_d
         if (h->class_count[k] == 0) { h->err = "a class has no points"; return ADMM_EINVAL; }
 
     const double t0 = now_ms();
-    // ---- S0: resident copies Phi [N][ldn] and Phi^T [n][ldN]
+    // ---- S0: Phi row-major [N][ldn] (setup), then the resident tile-major copies of Phi and Phi^T
+    const bool tc_path = h->opt.kernel_path == ADMM_PATH_TCGEN05;
+    const int64_t rtN = cdiv(N, kTileM), rtn = cdiv(n, kTileM), kbN = cdiv(N, kBlockK), kbn = cdiv(n, kBlockK);
+    if (std::max(rtN * kbn, rtn * kbN) * kTileM >= (1ll << 31)) { h->err = "Phi too large for 32-bit tile coordinates"; return ADMM_EINVAL; }
     ST_TRY(dev_alloc(h, &h->d_phi, N * h->ldn));
-    ST_TRY(dev_alloc(h, &h->d_phiT, n * h->ldN));
     ST_TRY(dev_alloc(h, &h->d_point_class, N));
     CU_TRY(h, cudaMemsetAsync(h->d_phi, 0, (size_t)N * h->ldn * 4, st));
-    CU_TRY(h, cudaMemsetAsync(h->d_phiT, 0, (size_t)n * h->ldN * 4, st));
     CU_TRY(h, cudaMemcpy2DAsync(h->d_phi, (size_t)h->ldn * 4, phi, (size_t)ld * 4, (size_t)n * 4, (size_t)N,
                                 phi_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
     CU_TRY(h, cudaMemcpyAsync(h->d_point_class, point_class, (size_t)N, cudaMemcpyHostToDevice, st));
     if (h->opt.storage == ADMM_STORAGE_FP32_TF32) launch_round_tf32(h->d_phi, N * h->ldn, st);
-    launch_transpose(h->d_phi, N, n, h->ldn, h->d_phiT, h->ldN, st);
+    if (tc_path) {
+        ST_TRY(dev_alloc(h, &h->d_phi_t, rtN * kbn * kTileM * kBlockK));
+        ST_TRY(dev_alloc(h, &h->d_phiT_t, rtn * kbN * kTileM * kBlockK));
+        launch_pack_tiles(h->d_phi, N, n, h->ldn, false, h->d_phi_t, st);
+        launch_pack_tiles(h->d_phi, N, n, h->ldn, true, h->d_phiT_t, st);
+    } else {
+        ST_TRY(dev_alloc(h, &h->d_phiT, n * h->ldN));
+        CU_TRY(h, cudaMemsetAsync(h->d_phiT, 0, (size_t)n * h->ldN * 4, st));
+        launch_transpose(h->d_phi, N, n, h->ldn, h->d_phiT, h->ldN, st);
+    }
     CU_TRY(h, cudaStreamSynchronize(st));
     const double t1 = now_ms();
 
@@ -309,6 +320,7 @@ static admm_status setup_impl(admm_handle* h, const float* phi, int32_t phi_on_d
     }
     launch_finish_S(h->d_Sinv, n, h->d_R, st);
     if (cudaStreamSynchronize(st) != cudaSuccess) { cleanup(); h->err = "S formation failed"; return ADMM_ECUDA; }
+    if (tc_path) { cudaFree(h->d_phi); h->d_phi = nullptr; }      // only the tile-major copies stay resident
     const double t2 = now_ms();
 
     // ---- S2: Cholesky + explicit inverse in fp64, shared by every plan and every rho (:222)

@@ -190,9 +190,10 @@ __global__ void __launch_bounds__(DRAIN ? 448 : 320, 1) admm_contract_kernel(con
                     tc::mbar_wait(&ctrl->empty[s], ph ^ 1);
                     tc::mbar_arrive_expect_tx(&ctrl->full[s], bytes);
                     const int k0 = (un.kb0 + kb) * kBlockK;
+                    const int trow = ((un.row0 >> 7) * L.big_kb_total + un.kb0 + kb) * kTileM;     // tile-major big operand
                     for (int b = 0; b < nbox; ++b)
-                        tc::tma_load_2d(stage_a_raw(s) + b * kBoxBytes, &L.map_big, &ctrl->full[s], k0,
-                                        un.row0 + b * kBoxRows, tc::kEvictFirst);
+                        tc::tma_load_2d(stage_a_raw(s) + b * kBoxBytes, &L.map_big, &ctrl->full[s], 0,
+                                        trow + b * kBoxRows, tc::kEvictFirst);
                     tc::tma_load_2d(stage_b_hi(s), &L.map_small_hi, &ctrl->full[s], k0, 0, tc::kEvictLast);
                     tc::tma_load_2d(stage_b_lo(s), &L.map_small_lo, &ctrl->full[s], k0, 0, tc::kEvictLast);
                     if (++s == n_stages) { s = 0; ph ^= 1; }
@@ -644,11 +645,10 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
             while (ia.u < unit_end || ib.u < unit_end) {
                 if (ia.u < unit_end && tc::mbar_test_wait(&ctrl->sa_empty[sa], pha ^ 1)) {
                     const TcUnit un = L.units[ia.u];
-                    // one 128-row box: rows past the end of the matrix are zero-filled by TMA, rows past the end of the
-                    // unit belong to a neighbouring unit and are ignored by the epilogue
+                    // one 16 KB tile of the tile-major big operand (rows past the end of the matrix are stored as zeros)
                     tc::mbar_arrive_expect_tx(&ctrl->sa_full[sa], kTileBytes);
-                    tc::tma_load_2d(a_ring + sa * kTileBytes, &L.map_big128, &ctrl->sa_full[sa], (un.kb0 + ia.kb) * kBlockK,
-                                    un.row0, tc::kEvictFirst);
+                    tc::tma_load_2d(a_ring + sa * kTileBytes, &L.map_big128, &ctrl->sa_full[sa], 0,
+                                    ((un.row0 >> 7) * L.big_kb_total + un.kb0 + ia.kb) * kTileM, tc::kEvictFirst);
                     ia.next(L, unit_end);
                     if (++sa == n_sa) { sa = 0; pha ^= 1; }
                 }

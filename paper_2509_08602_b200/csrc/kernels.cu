@@ -25,6 +25,39 @@ __global__ void transpose_kernel(const float* __restrict__ src, int64_t rows, in
     }
 }
 
+// Tile-major copy of a big operand for the tcgen05 contractions: dst[(rt * KB + kb)][128][32] = the 128 x 32 block of
+// rows rt*128.., columns kb*32.. of X (zero outside), X = src (TRANSPOSE = false) or src^T (true).  One TMA box of a
+// contraction kernel is then ONE contiguous 16 KB burst and a CTA walking k reads sequential memory: with the row-major
+// layout each box was 128 pieces of 128 B a row stride apart (1.8 MB for Phi^T at config 2: one DRAM page and one TLB
+// entry per piece).  Block = one tile, 256 threads.
+template <bool TRANSPOSE>
+__global__ void __launch_bounds__(256) pack_tiles_kernel(const float* __restrict__ src, int64_t src_rows, int64_t src_cols,
+                                                         int64_t ld_src, float* __restrict__ dst, int64_t KB) {
+    const int64_t kb = blockIdx.x, rt = blockIdx.y;
+    float* out = dst + ((rt * KB + kb) * kTileM) * kBlockK;
+    if (!TRANSPOSE) {
+        // X = src: rows rt*128 + r, cols kb*32 + c
+        for (int i = threadIdx.x; i < kTileM * kBlockK; i += 256) {
+            const int r = i >> 5, c = i & 31;
+            const int64_t row = rt * kTileM + r, col = kb * kBlockK + c;
+            out[i] = (row < src_rows && col < src_cols) ? src[row * ld_src + col] : 0.0f;
+        }
+    } else {
+        // X = src^T: X[j][i] = src[i][j]; tile rows j = rt*128 + r (src columns), tile cols i = kb*32 + c (src rows)
+        __shared__ float t[kBlockK][kTileM + 1];
+        for (int i = threadIdx.x; i < kTileM * kBlockK; i += 256) {
+            const int c = i >> 7, r = i & 127;                       // c: src row within the block, r: src column
+            const int64_t srow = kb * kBlockK + c, scol = rt * kTileM + r;
+            t[c][r] = (srow < src_rows && scol < src_cols) ? src[srow * ld_src + scol] : 0.0f;
+        }
+        __syncthreads();
+        for (int i = threadIdx.x; i < kTileM * kBlockK; i += 256) {
+            const int r = i >> 5, c = i & 31;
+            out[i] = t[c][r];
+        }
+    }
+}
+
 // out[r][j] = a_cls[class(row0 + r)] * phi[row0 + r][j]  in fp64 (operand of the fp64 SYRK)
 __global__ void scale_rows_kernel(const float* __restrict__ phi, int64_t ld, int64_t row0, int64_t rows, int64_t n,
                                   const uint8_t* __restrict__ cls, const double* __restrict__ a_cls, double* __restrict__ out) {
@@ -518,6 +551,16 @@ __global__ void gather_rows_kernel(const float* __restrict__ src, int64_t ld, co
 void launch_transpose(const float* src, int64_t rows, int64_t cols, int64_t ld_src, float* dst, int64_t ld_dst, cudaStream_t s) {
     dim3 grid((unsigned)cdiv(cols, 32), (unsigned)cdiv(rows, 32));
     transpose_kernel<<<grid, dim3(32, 8), 0, s>>>(src, rows, cols, ld_src, dst, ld_dst);
+}
+void launch_pack_tiles(const float* src, int64_t src_rows, int64_t src_cols, int64_t ld_src, bool transpose, float* dst,
+                       cudaStream_t s) {
+    if (!transpose) {
+        const int64_t KB = cdiv(src_cols, kBlockK), RT = cdiv(src_rows, kTileM);
+        pack_tiles_kernel<false><<<dim3((unsigned)KB, (unsigned)RT), 256, 0, s>>>(src, src_rows, src_cols, ld_src, dst, KB);
+    } else {
+        const int64_t KB = cdiv(src_rows, kBlockK), RT = cdiv(src_cols, kTileM);
+        pack_tiles_kernel<true><<<dim3((unsigned)KB, (unsigned)RT), 256, 0, s>>>(src, src_rows, src_cols, ld_src, dst, KB);
+    }
 }
 void launch_scale_rows_to_f64(const float* phi, int64_t ld, int64_t row0, int64_t rows, int64_t n, const uint8_t* cls,
                               const double* a_cls, double* out, cudaStream_t s) {

@@ -68,6 +68,7 @@ struct TcLaunch {
     int32_t grid;
     int32_t mma_passes;      // 3: 3xTF32 with on-chip split of the big operand; 2: big operand already on the tf32 grid
     int32_t epi;
+    int32_t n_sa, n_sb;      // fp32 kernel: depth of the big / small operand rings in shared memory
     int32_t chunk_kb;        // > 0: drain the TMEM accumulator every chunk_kb k-blocks (fp32 path, n_mma <= 128); 0: never
     EpiParams ep;
 };

@@ -562,9 +562,12 @@ struct CtrlF32 {
 __host__ __device__ inline int f32_b_bytes(int n_mma) { return 2 * n_mma * kBlockK * 4; }
 __host__ __device__ inline int f32_q_bytes(int n_mma) { return n_mma * kTileM * 4; }        // staged accumulator tile
 __host__ __device__ inline int f32_acc_bytes(int n_mma) { return 8 * n_mma * 8 * 4; }       // [8 warps][n_mma][8]
-// B ring: 3 stages (L2-resident operand, short latency); everything left goes to the A ring, whose depth is what
-// keeps enough HBM bytes in flight (ncu: with 4 x 16 KB the converter waited on TMA a third of the time)
-__host__ __device__ inline int f32_b_stages(int) { return 3; }
+// B ring: 4 stages when the A ring still gets 3 (measured at config 1: A depth 3..5 makes no difference, B depth 2 / 3 / 4
+// gives 120 / 107 / 104 us for K1: the L2-resident small operand arrives as 2 x n_mma rows of 128 B and has the longer latency)
+__host__ __device__ inline int f32_b_stages(int n_mma) {
+    const int fixed = 1024 + (int)sizeof(CtrlF32) + f32_q_bytes(n_mma) + f32_acc_bytes(n_mma);
+    return (fixed + 4 * f32_b_bytes(n_mma) + 3 * kTileBytes <= kSmemLimit) ? 4 : 3;
+}
 __host__ __device__ inline int f32_a_stages(int n_mma) {
     int s = (kSmemLimit - 1024 - (int)sizeof(CtrlF32) - f32_q_bytes(n_mma) - f32_acc_bytes(n_mma) -
              f32_b_stages(n_mma) * f32_b_bytes(n_mma)) / kTileBytes;
@@ -588,8 +591,8 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
     const int lane = threadIdx.x & 31;
     const int n_mma = L.ep.n_mma;
     const int bbytes = f32_b_bytes(n_mma);
-    const int n_sa = f32_a_stages(n_mma);
-    const int n_sb = f32_b_stages(n_mma);
+    const int n_sa = L.n_sa;
+    const int n_sb = L.n_sb;
     uint8_t* a_ring = smem;                                   // n_sa x 16 KB (1024-aligned)
     uint8_t* b_ring = smem + n_sa * kTileBytes;               // n_sb x bbytes (multiple of 1024: n_mma % 16 == 0)
     float* qs = reinterpret_cast<float*>(b_ring + n_sb * bbytes);
@@ -918,7 +921,9 @@ admm_status tc_launch(admm_handle* h, const TcLaunch& L) {
     if (L.mma_passes == 3) {
         if (n_mma > kF32MaxMmaN) { h->err = "tc_launch: the fp32 path needs n_mma <= 96"; return ADMM_EINVAL; }
         if (f32_a_stages(n_mma) < 2) { h->err = "tc_launch: fewer than 2 pipeline stages fit in shared memory"; return ADMM_EINVAL; }
-        admm_contract_f32_kernel<<<L.grid, kF32Threads, kSmemLimit, h->stream>>>(L);
+        TcLaunch L2 = L;
+        L2.n_sb = f32_b_stages(n_mma); L2.n_sa = f32_a_stages(n_mma);
+        admm_contract_f32_kernel<<<L.grid, kF32Threads, kSmemLimit, h->stream>>>(L2);
     } else {
         admm_contract_kernel<false><<<L.grid, 320, kSmemLimit, h->stream>>>(L);
     }

@@ -53,7 +53,7 @@ typedef struct {
 enum {
     ADMM_STORAGE_FP32_3XTF32 = 0, /* fp32 storage, hi/lo split on chip, 3 tf32 MMAs: the fp32 path (1e-4 parity) */
     ADMM_STORAGE_FP32_TF32   = 1, /* Phi rounded once to tf32 (kept in an fp32 container), 2 tf32 MMAs */
-    ADMM_STORAGE_BF16        = 2, /* Phi rounded once to bf16, bf16 MMAs (1e-2 parity)  [not built yet] */
+    ADMM_STORAGE_BF16        = 2, /* Phi rounded once to bf16 (half the HBM bytes), plan operands as bf16 hi/lo pairs, 2 bf16 MMAs (1e-2 parity) */
     ADMM_STORAGE_CSR         = 3  /* thresholded CSR                                     [not built yet] */
 };
 

@@ -50,8 +50,9 @@ struct EpiParams {
     float sense[kMaxClasses];
     float thr[kMaxClasses];
     float* s1;                      // [Bpad][ldN] single state s = x + y of block 1
-    float* g_hi;                    // [Bpad][ldN] operand of K1: tf32 head of a (2 z1 - s1 - c/rho)
-    float* g_lo;                    // [Bpad][ldN] tail
+    void* g_hi;                     // [Bpad][ldN] operand of K1: head of a (2 z1 - s1 - c/rho): fp32 on the tf32 grid, or bf16
+    void* g_lo;                     // [Bpad][ldN] tail
+    int32_t small_bf16;             // 1: the small operands (G, V, T) are emitted as bf16 hi/lo pairs (ADMM_STORAGE_BF16)
     float* resid_partial;           // [grid][kMaxBpad][kNumResid] per-CTA residual sums (nullptr: not this iteration)
     double* hinge_partial;          // objective: [grid][kMaxBpad][kMaxClasses]
     float* qraw;                    // EPI_RAW (test hook): raw accumulators [slot][ldN]
@@ -68,6 +69,8 @@ struct TcLaunch {
     int32_t grid;
     int32_t mma_passes;      // 3: 3xTF32 with on-chip split of the big operand; 2: big operand already on the tf32 grid
     int32_t epi;
+    int32_t kblk;            // elements per k-block = per 128-byte row: 32 (fp32 / tf32) or 64 (bf16)
+    int32_t mma_kind;        // 0: kind::tf32, 1: kind::f16 with bf16 operands
     int32_t n_sa, n_sb;      // fp32 kernel: depth of the big / small operand rings in shared memory
     int32_t chunk_kb;        // > 0: drain the TMEM accumulator every chunk_kb k-blocks (fp32 path, n_mma <= 128); 0: never
     EpiParams ep;
@@ -97,6 +100,7 @@ struct admm_handle {
     double* d_R = nullptr;         // [n]
     double* d_Sinv = nullptr;      // [n][lds], lds = n rounded up to even (16-byte rows for cp.async), pad = 0
     int64_t lds = 0;
+    int kblk = 32;                 // elements per 128-byte k-block of the stored Phi: 32 (fp32) or 64 (bf16 storage)
     int k2_wj = 1;                 // K2b block tile = 16 * k2_wj rows (chosen when the batch buffers are allocated)
     std::vector<double> h_R;
 
@@ -136,11 +140,13 @@ struct admm_handle {
 // ---- gemm_tc.cu
 admm_status tc_init(admm_handle* h);                       // resolves cuTensorMapEncodeTiled, sets smem attribute
 admm_status tc_make_map(admm_handle* h, CUtensorMap* out, const void* base, int64_t rows, int64_t cols,
-                        int64_t ld_elems, int box_rows);
+                        int64_t ld_elems, int box_rows, int elem_bytes = 4);
 admm_status tc_launch(admm_handle* h, const TcLaunch& L);
 
 // ---- kernels.cu  (everything that is not a tcgen05 contraction)
 void launch_pack_tiles(const float* src, int64_t src_rows, int64_t src_cols, int64_t ld_src, bool transpose, float* dst, cudaStream_t s);
+void launch_pack_tiles_bf16(const float* src, int64_t src_rows, int64_t src_cols, int64_t ld_src, bool transpose, void* dst, cudaStream_t s);
+void launch_round_bf16(float* x, int64_t count, cudaStream_t s);
 void launch_transpose(const float* src, int64_t rows, int64_t cols, int64_t ld_src, float* dst, int64_t ld_dst, cudaStream_t s);
 void launch_scale_rows_to_f64(const float* phi, int64_t ld, int64_t row0, int64_t rows, int64_t n,
                               const uint8_t* cls, const double* a_cls, double* out, cudaStream_t s);
@@ -155,11 +161,11 @@ void launch_k2b(admm_handle* h, int Bact, bool resid, cudaStream_t s);
 void launch_simt_k1(admm_handle* h, int slot0, int nact, int n_mma, int splits, cudaStream_t s);
 void launch_simt_k3(admm_handle* h, const EpiParams& ep, int epi, const float* vhi, const float* vlo, float* qbuf, cudaStream_t s);
 void launch_convergence(admm_handle* h, int Bact, int grid1, int grid2, float tol, float eps_abs, cudaStream_t s);
-void launch_make_t(admm_handle* h, int Bact, float* t_hi, float* t_lo, float* t_f32, cudaStream_t s);
+void launch_make_t(admm_handle* h, int Bact, void* t_hi, void* t_lo, float* t_f32, cudaStream_t s);
 void launch_objective_reduce(admm_handle* h, int B, int grid, const float* t_f32, const double* wnorm, double* obj_slot, cudaStream_t s);
 void launch_gather_rows(const float* src, int64_t ld, const int32_t* plan_slot, int B, int64_t n, float* dst, cudaStream_t s);
 void launch_state_out(admm_handle* h, const EpiParams& ep, int slot, double beta, float* z1, float* y1, double* z2, double* y2, cudaStream_t s);
 int k2b_grid(const admm_handle* h, int Bact);
 int k2_choose_wj(const admm_handle* h, int Bpad);
-void launch_split_tf32(const float* x, int64_t count, float* hi, float* lo, cudaStream_t s);
+void launch_split_small(const float* x, int64_t count, int64_t ld, void* hi, void* lo, bool bf16, cudaStream_t s);
 void launch_reduce_partial(admm_handle* h, int nact, int n_mma, double* out, cudaStream_t s);

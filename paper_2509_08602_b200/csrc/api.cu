@@ -59,10 +59,10 @@ bool is_device_ptr(const void* p) {
 
 // ---- unit tables ------------------------------------------------------------------------------------------
 // K3: the 128-row tiles of Phi (aligned: the big operand is stored tile-major) are dealt evenly to the CTAs.
-void build_units_k3(int64_t N, int64_t n, int sm, std::vector<TcUnit>& units, std::vector<int32_t>& begin) {
+void build_units_k3(int64_t N, int64_t n, int sm, int kblk, std::vector<TcUnit>& units, std::vector<int32_t>& begin) {
     const int64_t tiles = cdiv(N, kTileM);
     const int grid = (int)std::min<int64_t>(sm, tiles);
-    const int kb = (int)cdiv(n, kBlockK);
+    const int kb = (int)cdiv(n, kblk);
     units.clear(); begin.assign(1, 0);
     for (int c = 0; c < grid; ++c) {
         for (int64_t t = tiles * c / grid; t < tiles * (c + 1) / grid; ++t) {
@@ -78,12 +78,12 @@ void build_units_k3(int64_t N, int64_t n, int sm, std::vector<TcUnit>& units, st
 // units).  All CTAs are inside the same slab at the same time, so G is read from HBM once per iteration instead of once
 // per m-tile (measured at config 2 before this ordering: K1 took 7.6 ms against K3's 4.8 ms for the same Phi bytes).
 // Every unit writes its own partial-sum slot; the slots of one m-tile are numbered contiguously (mtile_slot_begin).
-void build_units_k1(int64_t N, int64_t n, int sm, int n_mma_max, int slab_kb, std::vector<TcUnit>& units,
+void build_units_k1(int64_t N, int64_t n, int sm, int kblk, int n_mma_max, int slab_kb, std::vector<TcUnit>& units,
                     std::vector<int32_t>& begin, std::vector<int32_t>& mtile_slot_begin) {
     const int64_t T = cdiv(n, kTileM);
-    const int64_t KB = cdiv(N, kBlockK);
+    const int64_t KB = cdiv(N, kblk);
     const int grid = (int)std::min<int64_t>(sm, T * std::max<int64_t>(1, KB / 8));
-    const int64_t g_bytes_per_kb = (int64_t)2 * n_mma_max * kBlockK * 4;
+    const int64_t g_bytes_per_kb = (int64_t)2 * n_mma_max * 128;      // hi + lo rows of 128 bytes
     int64_t slabs = 1;
     if (slab_kb > 0) slabs = cdiv(KB, slab_kb);
     else if (KB * g_bytes_per_kb > (64ll << 20)) slabs = cdiv(KB * g_bytes_per_kb, 32ll << 20);
@@ -171,10 +171,11 @@ EpiParams base_epi(admm_handle* h) {
     }
     ep.s1 = h->d_s1; ep.g_hi = h->d_ghi; ep.g_lo = h->d_glo;
     ep.resid_partial = nullptr; ep.hinge_partial = h->d_hinge;
+    ep.small_bf16 = h->opt.storage == ADMM_STORAGE_BF16 ? 1 : 0;
     return ep;
 }
 
-int mma_passes(const admm_handle* h) { return h->opt.storage == ADMM_STORAGE_FP32_TF32 ? 2 : 3; }
+int mma_passes(const admm_handle* h) { return h->opt.storage == ADMM_STORAGE_FP32_3XTF32 ? 3 : 2; }
 // fp32 path: drain the hi.hi TMEM accumulator every k-block (32 elements of K, 4 MMAs) -- see gemm_tc.cu
 int chunk_kb(const admm_handle* h) {
     if (h->opt.storage != ADMM_STORAGE_FP32_3XTF32 || h->opt.kernel_path != ADMM_PATH_TCGEN05) return 0;
@@ -193,14 +194,18 @@ admm_status contract(admm_handle* h, int epi, int slot0, int nact, const float* 
     TcLaunch L{};
     const bool k1 = (epi == EPI_K1_PARTIAL);
     const int64_t big_rows = k1 ? h->n : h->N, big_cols = k1 ? h->N : h->n, big_ld = k1 ? h->ldN : h->ldn;
-    // big operand: tile-major [row tiles][k-blocks][128][32] seen as a 2-D tensor of 128-byte rows
-    const int64_t kb_total = cdiv(big_cols, kBlockK), tiled_rows = cdiv(big_rows, kTileM) * kb_total * kTileM;
-    ST_TRY(tc_make_map(h, &L.map_big, k1 ? h->d_phiT_t : h->d_phi_t, tiled_rows, kBlockK, kBlockK, kBoxRows));
-    ST_TRY(tc_make_map(h, &L.map_big128, k1 ? h->d_phiT_t : h->d_phi_t, tiled_rows, kBlockK, kBlockK, kTileM));
+    // big operand: tile-major [row tiles][k-blocks][128 rows][128 bytes] seen as a 2-D tensor of 128-byte rows
+    const bool bf16 = h->opt.storage == ADMM_STORAGE_BF16;
+    const int eb = bf16 ? 2 : 4, kblk = h->kblk;
+    const int64_t kb_total = cdiv(big_cols, kblk), tiled_rows = cdiv(big_rows, kTileM) * kb_total * kTileM;
+    ST_TRY(tc_make_map(h, &L.map_big, k1 ? h->d_phiT_t : h->d_phi_t, tiled_rows, kblk, kblk, kBoxRows, eb));
+    ST_TRY(tc_make_map(h, &L.map_big128, k1 ? h->d_phiT_t : h->d_phi_t, tiled_rows, kblk, kblk, kTileM, eb));
     L.big_kb_total = (int32_t)kb_total;
-    // the small operand has Bpad rows allocated; rows >= nact of the box are dead columns of D
-    ST_TRY(tc_make_map(h, &L.map_small_hi, small_hi + (int64_t)slot0 * big_ld, h->Bpad - slot0, big_cols, big_ld, n_mma));
-    ST_TRY(tc_make_map(h, &L.map_small_lo, small_lo + (int64_t)slot0 * big_ld, h->Bpad - slot0, big_cols, big_ld, n_mma));
+    L.kblk = kblk; L.mma_kind = bf16 ? 1 : 0;
+    // the small operand has Bpad rows allocated (row pitch big_ld * 4 bytes whatever the element type); rows >= nact of the
+    // box are dead columns of D
+    ST_TRY(tc_make_map(h, &L.map_small_hi, small_hi + (int64_t)slot0 * big_ld, h->Bpad - slot0, big_cols, bf16 ? 2 * big_ld : big_ld, n_mma, eb));
+    ST_TRY(tc_make_map(h, &L.map_small_lo, small_lo + (int64_t)slot0 * big_ld, h->Bpad - slot0, big_cols, bf16 ? 2 * big_ld : big_ld, n_mma, eb));
     L.units = k1 ? h->d_units_k1 : h->d_units_k3;
     L.cta_unit_begin = k1 ? h->d_cta_begin_k1 : h->d_cta_begin_k3;
     L.grid = k1 ? h->grid_k1 : h->grid_k3;
@@ -272,7 +277,9 @@ static admm_status setup_impl(admm_handle* h, const float* phi, int32_t phi_on_d
     const double t0 = now_ms();
     // ---- S0: Phi row-major [N][ldn] (setup), then the resident tile-major copies of Phi and Phi^T
     const bool tc_path = h->opt.kernel_path == ADMM_PATH_TCGEN05;
-    const int64_t rtN = cdiv(N, kTileM), rtn = cdiv(n, kTileM), kbN = cdiv(N, kBlockK), kbn = cdiv(n, kBlockK);
+    const bool bf16 = h->opt.storage == ADMM_STORAGE_BF16;
+    h->kblk = bf16 ? 64 : kBlockK;
+    const int64_t rtN = cdiv(N, kTileM), rtn = cdiv(n, kTileM), kbN = cdiv(N, h->kblk), kbn = cdiv(n, h->kblk);
     if (std::max(rtN * kbn, rtn * kbN) * kTileM >= (1ll << 31)) { h->err = "Phi too large for 32-bit tile coordinates"; return ADMM_EINVAL; }
     ST_TRY(dev_alloc(h, &h->d_phi, N * h->ldn));
     ST_TRY(dev_alloc(h, &h->d_point_class, N));
@@ -280,12 +287,20 @@ static admm_status setup_impl(admm_handle* h, const float* phi, int32_t phi_on_d
     CU_TRY(h, cudaMemcpy2DAsync(h->d_phi, (size_t)h->ldn * 4, phi, (size_t)ld * 4, (size_t)n * 4, (size_t)N,
                                 phi_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
     CU_TRY(h, cudaMemcpyAsync(h->d_point_class, point_class, (size_t)N, cudaMemcpyHostToDevice, st));
+    // reduced storage: Phi is rounded ONCE here, so S below is formed from the matrix the kernels consume (SURVEY H-c)
     if (h->opt.storage == ADMM_STORAGE_FP32_TF32) launch_round_tf32(h->d_phi, N * h->ldn, st);
+    if (bf16) launch_round_bf16(h->d_phi, N * h->ldn, st);
     if (tc_path) {
+        // every tile is 128 rows x 128 bytes = 16 KB = 4096 floats, whatever the element type
         ST_TRY(dev_alloc(h, &h->d_phi_t, rtN * kbn * kTileM * kBlockK));
         ST_TRY(dev_alloc(h, &h->d_phiT_t, rtn * kbN * kTileM * kBlockK));
-        launch_pack_tiles(h->d_phi, N, n, h->ldn, false, h->d_phi_t, st);
-        launch_pack_tiles(h->d_phi, N, n, h->ldn, true, h->d_phiT_t, st);
+        if (bf16) {
+            launch_pack_tiles_bf16(h->d_phi, N, n, h->ldn, false, h->d_phi_t, st);
+            launch_pack_tiles_bf16(h->d_phi, N, n, h->ldn, true, h->d_phiT_t, st);
+        } else {
+            launch_pack_tiles(h->d_phi, N, n, h->ldn, false, h->d_phi_t, st);
+            launch_pack_tiles(h->d_phi, N, n, h->ldn, true, h->d_phiT_t, st);
+        }
     } else {
         ST_TRY(dev_alloc(h, &h->d_phiT, n * h->ldN));
         CU_TRY(h, cudaMemsetAsync(h->d_phiT, 0, (size_t)n * h->ldN * 4, st));
@@ -365,14 +380,14 @@ static admm_status setup_impl(admm_handle* h, const float* phi, int32_t phi_on_d
     // ---- work decomposition of the two contractions
     ST_TRY(tc_init(h));
     std::vector<TcUnit> u; std::vector<int32_t> b, msb;
-    build_units_k3(N, n, h->sm_count, u, b);
+    build_units_k3(N, n, h->sm_count, h->kblk, u, b);
     h->grid_k3 = (int)b.size() - 1;
     ST_TRY(dev_alloc(h, &h->d_units_k3, (int64_t)u.size()));
     ST_TRY(dev_alloc(h, &h->d_cta_begin_k3, (int64_t)b.size()));
     CU_TRY(h, cudaMemcpy(h->d_units_k3, u.data(), u.size() * sizeof(TcUnit), cudaMemcpyHostToDevice));
     CU_TRY(h, cudaMemcpy(h->d_cta_begin_k3, b.data(), b.size() * 4, cudaMemcpyHostToDevice));
     if (h->opt.kernel_path == ADMM_PATH_TCGEN05) {
-        build_units_k1(N, n, h->sm_count, h->opt.storage == ADMM_STORAGE_FP32_3XTF32 ? 96 : kMaxMmaN, h->opt.k1_slab_kb, u, b, msb);
+        build_units_k1(N, n, h->sm_count, h->kblk, h->opt.storage == ADMM_STORAGE_FP32_3XTF32 ? 96 : kMaxMmaN, h->opt.k1_slab_kb, u, b, msb);
         h->grid_k1 = (int)b.size() - 1;
         h->slots_k1 = msb.back();
     } else {
@@ -411,8 +426,11 @@ admm_status admm_setup(admm_handle** out, const float* phi, int32_t phi_on_devic
     if (opt) o = *opt; else admm_default_options(&o);
     if (o.check_every <= 0) o.check_every = 10;
     if (!(o.eps_abs > 0.f)) o.eps_abs = 1e-6f;
-    if (o.storage != ADMM_STORAGE_FP32_3XTF32 && o.storage != ADMM_STORAGE_FP32_TF32) {
-        g_setup_err = "storage mode not built yet (only FP32_3XTF32 and FP32_TF32)"; return ADMM_EINVAL;
+    if (o.storage != ADMM_STORAGE_FP32_3XTF32 && o.storage != ADMM_STORAGE_FP32_TF32 && o.storage != ADMM_STORAGE_BF16) {
+        g_setup_err = "storage mode not built yet (FP32_3XTF32, FP32_TF32 and BF16 are)"; return ADMM_EINVAL;
+    }
+    if (o.storage == ADMM_STORAGE_BF16 && o.kernel_path != ADMM_PATH_TCGEN05) {
+        g_setup_err = "ADMM_STORAGE_BF16 exists on the tcgen05 path only"; return ADMM_EINVAL;
     }
     if (o.kernel_path != ADMM_PATH_TCGEN05 && o.kernel_path != ADMM_PATH_SIMT) { g_setup_err = "unknown kernel_path"; return ADMM_EINVAL; }
     admm_handle* h = new (std::nothrow) admm_handle();
@@ -733,7 +751,7 @@ admm_status admm_contract_probe(admm_handle* h, int32_t which, int32_t B, const 
     ST_TRY(dev_alloc(h, &stage, (int64_t)h->Bpad * ldK)); g.a = stage;
     CU_TRY(h, cudaMemsetAsync(stage, 0, (size_t)h->Bpad * ldK * 4, st));
     CU_TRY(h, cudaMemcpy2DAsync(stage, (size_t)ldK * 4, small, (size_t)K * 4, (size_t)K * 4, (size_t)B, cudaMemcpyHostToDevice, st));
-    launch_split_tf32(stage, (int64_t)h->Bpad * ldK, hi, lo, st);
+    launch_split_small(stage, (int64_t)h->Bpad * ldK, ldK, hi, lo, h->opt.storage == ADMM_STORAGE_BF16, st);
     const int n_mma = (int)round_up(B, 16);
     if (which == 0) {
         if (simt) launch_simt_k1(h, 0, B, n_mma, h->grid_k1, st);

@@ -8,11 +8,40 @@
 // The operand of the next A r1 product is r1 = z1+ - y1+ - c/rho = 2 z1+ - s1+ - c/rho, scaled by a_i.
 #pragma once
 #include <cuda_runtime.h>
+#include <cuda_bf16.h>
 #include "tc_ptx.cuh"
+
+// A small-operand element x as a hi/lo pair for the tensor cores: fp32 containers on the tf32 grid (hi = rna(x),
+// lo = rna(x - hi): 21 bits kept, both rounded here so the hardware's operand truncation never bites), or a bf16
+// pair (16 bits kept) for ADMM_STORAGE_BF16.
+__device__ __forceinline__ void emit_small(void* hi, void* lo, int64_t rowbase, int64_t col, float x, bool bf16) {
+    const int64_t idx = (bf16 ? 2 * rowbase : rowbase) + col;      // same row pitch in bytes for both element types
+    if (bf16) {
+        const __nv_bfloat16 h = __float2bfloat16_rn(x);
+        reinterpret_cast<__nv_bfloat16*>(hi)[idx] = h;
+        reinterpret_cast<__nv_bfloat16*>(lo)[idx] = __float2bfloat16_rn(x - __bfloat162float(h));
+    } else {
+        const float h = tc::tf32_rna(x);
+        reinterpret_cast<float*>(hi)[idx] = h;
+        reinterpret_cast<float*>(lo)[idx] = tc::tf32_rna(x - h);
+    }
+}
+__device__ __forceinline__ void emit_small(void* hi, void* lo, int64_t rowbase, int64_t col, double x, bool bf16) {
+    const int64_t idx = (bf16 ? 2 * rowbase : rowbase) + col;
+    if (bf16) {
+        const __nv_bfloat16 h = __float2bfloat16_rn((float)x);
+        reinterpret_cast<__nv_bfloat16*>(hi)[idx] = h;
+        reinterpret_cast<__nv_bfloat16*>(lo)[idx] = __float2bfloat16_rn((float)(x - (double)__bfloat162float(h)));
+    } else {
+        const float h = tc::tf32_rn((float)x);
+        reinterpret_cast<float*>(hi)[idx] = h;
+        reinterpret_cast<float*>(lo)[idx] = tc::tf32_rn((float)(x - (double)h));
+    }
+}
 
 struct Epi1Out {
     float s_new;
-    float g_hi, g_lo;
+    float g;          // operand of the next A r1 product, before the hi/lo split (emit_small)
 };
 
 // one (point, plan) element of epilogue-1.  acc[0..4] += residual terms when `resid`.
@@ -23,8 +52,7 @@ __device__ __forceinline__ Epi1Out epi1_element(float s_old, float q, float a, f
     float g = a * (2.0f * z_new - s_new - cr);
     Epi1Out o;
     o.s_new = s_new;
-    o.g_hi = tc::tf32_rna(g);
-    o.g_lo = tc::tf32_rna(g - o.g_hi);      // rounded here: the tensor core would otherwise cut lo's low bits toward zero
+    o.g = g;
     if (resid) {
         float y_old = s_old - z_old;
         float y_new = s_new - z_new;

@@ -101,8 +101,7 @@ __device__ __noinline__ void epi_cols16(const TcLaunch& L, const EpiCtx& cx, int
                 Epi1Out o = epi1_element(so[jj], q[jj], cx.a_k, cr, ub, cx.resid, racc);
                 const int64_t idx = (int64_t)(ep.slot0 + p) * ep.ldN + cx.row;
                 ep.s1[idx] = o.s_new;
-                ep.g_hi[idx] = o.g_hi;
-                ep.g_lo[idx] = o.g_lo;
+                emit_small(ep.g_hi, ep.g_lo, (int64_t)(ep.slot0 + p) * ep.ldN, cx.row, o.g, ep.small_bf16 != 0);
             } else {
                 hinge = on ? fmaxf(0.0f, cx.sense * (cx.thr - q[jj])) : 0.0f;
             }
@@ -189,7 +188,7 @@ __global__ void __launch_bounds__(DRAIN ? 448 : 320, 1) admm_contract_kernel(con
                 for (int kb = 0; kb < un.kb_count; ++kb) {
                     tc::mbar_wait(&ctrl->empty[s], ph ^ 1);
                     tc::mbar_arrive_expect_tx(&ctrl->full[s], bytes);
-                    const int k0 = (un.kb0 + kb) * kBlockK;
+                    const int k0 = (un.kb0 + kb) * L.kblk;
                     const int trow = ((un.row0 >> 7) * L.big_kb_total + un.kb0 + kb) * kTileM;     // tile-major big operand
                     for (int b = 0; b < nbox; ++b)
                         tc::tma_load_2d(stage_a_raw(s) + b * kBoxBytes, &L.map_big, &ctrl->full[s], 0,
@@ -203,7 +202,8 @@ __global__ void __launch_bounds__(DRAIN ? 448 : 320, 1) admm_contract_kernel(con
     } else if (warp == 1) {
         // ------------------------------------------------------------ UMMA issuer
         if (lane == 0) {
-            const uint32_t idesc = tc::umma_idesc(2u, kTileM, (uint32_t)n_mma);
+            const bool bf16 = L.mma_kind == 1;
+            const uint32_t idesc = tc::umma_idesc(bf16 ? 1u : 2u, kTileM, (uint32_t)n_mma);
             int s = 0; uint32_t ph = 0;
             int a = 0; uint32_t aph = 0;
             int b = 0; uint32_t bph = 0;
@@ -241,6 +241,10 @@ __global__ void __launch_bounds__(DRAIN ? 448 : 320, 1) admm_contract_kernel(con
                                     tc::umma_tf32(d_small, a_raw + koff, b_lo + koff, idesc, first_u);
                                 }
                                 tc::umma_tf32(d_tmem, a_raw + koff, b_hi + koff, idesc, first);
+                            } else if (bf16) {
+                                // bf16 storage: Phi is exact in bf16, the plan operand is a bf16 hi/lo pair; 16 elements per k-step
+                                tc::umma_f16(d_tmem, a_raw + koff, b_lo + koff, idesc, first);
+                                tc::umma_f16(d_tmem, a_raw + koff, b_hi + koff, idesc, 1u);
                             } else {
                                 if (passes == 3) {
                                     tc::umma_tf32(d_tmem, a_lo + koff, b_hi + koff, idesc, first);
@@ -454,8 +458,8 @@ __device__ __noinline__ void epilogue_unit_t(const TcLaunch& L, const TcUnit& un
     const uint32_t ldN = (uint32_t)ep.ldN;                     // Bpad * ldN < 2^32 (checked on the host)
     const int64_t base = (int64_t)ep.slot0 * ep.ldN + row;
     float* s1p = ep.s1 + base;
-    float* ghp = ep.g_hi + base;
-    float* glp = ep.g_lo + base;
+    float* ghp = reinterpret_cast<float*>(ep.g_hi) + base;       // fp32 path only (this kernel)
+    float* glp = reinterpret_cast<float*>(ep.g_lo) + base;
     constexpr int PB = 8;
     for (int p0 = p_begin; p0 < p_end; p0 += PB) {
         float so[PB], ub[PB], cr[PB];
@@ -483,8 +487,9 @@ __device__ __noinline__ void epilogue_unit_t(const TcLaunch& L, const TcUnit& un
                     Epi1Out o = epi1_element(so[j], q, a_k, cr[j], on ? ub[j] : 0.0f, RESID, racc);
                     const uint32_t off = (uint32_t)p * ldN;
                     s1p[off] = o.s_new;
-                    ghp[off] = o.g_hi;
-                    glp[off] = o.g_lo;
+                    const float ghi = tc::tf32_rna(o.g);
+                    ghp[off] = ghi;
+                    glp[off] = tc::tf32_rna(o.g - ghi);
                 } else {
                     hinge = on ? fmaxf(0.0f, sense * (thr - q)) : 0.0f;
                 }
@@ -888,14 +893,14 @@ admm_status tc_init(admm_handle* h) {
 // 2-D fp32 tensor [rows][cols] with row stride ld_elems, box = {32 cols (128 B), box_rows}, 128-byte swizzle,
 // out-of-bounds elements read as zero.
 admm_status tc_make_map(admm_handle* h, CUtensorMap* out, const void* base, int64_t rows, int64_t cols,
-                        int64_t ld_elems, int box_rows) {
+                        int64_t ld_elems, int box_rows, int elem_bytes) {
     cuuint64_t gdim[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
-    cuuint64_t gstride[1] = {(cuuint64_t)ld_elems * 4};
-    cuuint32_t box[2] = {(cuuint32_t)kBlockK, (cuuint32_t)box_rows};
+    cuuint64_t gstride[1] = {(cuuint64_t)ld_elems * elem_bytes};
+    cuuint32_t box[2] = {(cuuint32_t)(128 / elem_bytes), (cuuint32_t)box_rows};       // 128-byte rows
     cuuint32_t estr[2] = {1, 1};
-    CUresult r = g_encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(base), gdim, gstride, box, estr,
-                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    CUresult r = g_encode(out, elem_bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
+                          const_cast<void*>(base), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                          CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         char buf[160];
         snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (%d) rows=%lld cols=%lld ld=%lld box_rows=%d", (int)r,

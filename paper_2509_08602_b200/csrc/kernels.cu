@@ -72,6 +72,40 @@ __global__ void round_tf32_kernel(float* x, int64_t count) {
     if (i < count) x[i] = tc::tf32_rn(x[i]);
 }
 
+__global__ void round_bf16_kernel(float* x, int64_t count) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < count) x[i] = __bfloat162float(__float2bfloat16_rn(x[i]));
+}
+
+// bf16 tile-major copy: dst[(rt * KB + kb)][128][64] bf16 (128-byte rows of 64 elements); src holds values already on
+// the bf16 grid (round_bf16_kernel), so the conversion is exact.
+template <bool TRANSPOSE>
+__global__ void __launch_bounds__(256) pack_tiles_bf16_kernel(const float* __restrict__ src, int64_t src_rows, int64_t src_cols,
+                                                              int64_t ld_src, __nv_bfloat16* __restrict__ dst, int64_t KB) {
+    constexpr int KE = 64;
+    const int64_t kb = blockIdx.x, rt = blockIdx.y;
+    __nv_bfloat16* out = dst + ((rt * KB + kb) * kTileM) * KE;
+    if (!TRANSPOSE) {
+        for (int i = threadIdx.x; i < kTileM * KE; i += 256) {
+            const int r = i >> 6, c = i & 63;
+            const int64_t row = rt * kTileM + r, col = kb * KE + c;
+            out[i] = __float2bfloat16_rn((row < src_rows && col < src_cols) ? src[row * ld_src + col] : 0.0f);
+        }
+    } else {
+        __shared__ float t[KE][kTileM + 1];
+        for (int i = threadIdx.x; i < kTileM * KE; i += 256) {
+            const int c = i >> 7, r = i & 127;
+            const int64_t srow = kb * KE + c, scol = rt * kTileM + r;
+            t[c][r] = (srow < src_rows && scol < src_cols) ? src[srow * ld_src + scol] : 0.0f;
+        }
+        __syncthreads();
+        for (int i = threadIdx.x; i < kTileM * KE; i += 256) {
+            const int r = i >> 6, c = i & 63;
+            out[i] = __float2bfloat16_rn(t[c][r]);
+        }
+    }
+}
+
 // R_j = 1/sqrt(M_jj) (1 if the row of A D is zero)
 __global__ void make_R_kernel(const double* __restrict__ M, int64_t n, double* __restrict__ R) {
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -133,9 +167,7 @@ __global__ void emit_g_kernel(const EpiParams ep, int Bact) {
     float s = ep.s1[(int64_t)p * ep.ldN + i];
     float z = fminf(fmaxf(s, 0.f), ub);
     float g = ep.a_cls[cls] * (2.f * z - s - cr);
-    float hi = tc::tf32_rna(g);
-    ep.g_hi[(int64_t)p * ep.ldN + i] = hi;
-    ep.g_lo[(int64_t)p * ep.ldN + i] = tc::tf32_rna(g - hi);
+    emit_small(ep.g_hi, ep.g_lo, (int64_t)p * ep.ldN, i, g, ep.small_bf16 != 0);
 }
 
 __global__ void state_out_kernel(const EpiParams ep, int slot, const double* __restrict__ s2, const double* __restrict__ R,
@@ -160,17 +192,14 @@ __global__ void state_out_kernel(const EpiParams ep, int slot, const double* __r
 // t = rho R max(s2 - R beta, 0): fp32 output + tf32 hi/lo operand of the objective contraction
 __global__ void make_t_kernel(const double* __restrict__ s2, const double* __restrict__ R, const double* __restrict__ beta,
                               const double* __restrict__ rho, int64_t n, int64_t ldn, int Bact,
-                              float* __restrict__ t_hi, float* __restrict__ t_lo, float* __restrict__ t_f32) {
+                              void* __restrict__ t_hi, void* __restrict__ t_lo, float* __restrict__ t_f32, int bf16) {
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int p = blockIdx.y;
     if (j >= n || p >= Bact) return;
     double y2 = fmax(s2[(int64_t)p * ldn + j] - R[j] * beta[p], 0.0);
     double t = rho[p] * R[j] * y2;
-    float tf = (float)t;
-    float hi = tc::tf32_rn(tf);
-    t_hi[(int64_t)p * ldn + j] = hi;
-    t_lo[(int64_t)p * ldn + j] = tc::tf32_rn((float)(t - (double)hi));
-    t_f32[(int64_t)p * ldn + j] = tf;
+    emit_small(t_hi, t_lo, (int64_t)p * ldn, j, t, bf16 != 0);
+    t_f32[(int64_t)p * ldn + j] = (float)t;
 }
 
 // ------------------------------------------------------------------------------------------ K2a: rhs of Eq. (6)
@@ -223,7 +252,7 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
                                                   const double* __restrict__ rhs, double* __restrict__ s2,
                                                   const double* __restrict__ R, const double* __restrict__ beta,
                                                   int64_t n, int64_t ldn, int Bact,
-                                                  float* __restrict__ v_hi, float* __restrict__ v_lo,
+                                                  void* __restrict__ v_hi, void* __restrict__ v_lo, int bf16,
                                                   double* __restrict__ resid_partial) {
     // 8 warps = WJ row groups x 2 plan halves x KS k-slices (a lone warp per scheduler cannot hide the DMMA issue
     // latency: measured 14 % pipe utilisation with 2 warps per block); the k-slices are summed through shared memory.
@@ -341,9 +370,7 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
                     const double z_new = fmin(s_new, bh);                 // (4b)
                     s2[(int64_t)p * ldn + j] = s_new;
                     const double rv = R[j] * v;
-                    const float hi = tc::tf32_rn((float)rv);
-                    v_hi[(int64_t)p * ldn + j] = hi;
-                    v_lo[(int64_t)p * ldn + j] = tc::tf32_rn((float)(rv - (double)hi));
+                    emit_small(v_hi, v_lo, (int64_t)p * ldn, j, rv, bf16 != 0);
                     if (resid) {
                         const double y_old = s_old - z_old, y_new = s_new - z_new, x = s_new - y_old;
                         ra[0] += (x - z_new) * (x - z_new);
@@ -474,7 +501,7 @@ __global__ void __launch_bounds__(128) simt_epilogue_kernel(const EpiParams ep, 
                 float cr = ep.crtab[cls * kMaxBpad + p];
                 int64_t idx = (int64_t)p * ep.ldN + row;
                 Epi1Out o = epi1_element(ep.s1[idx], q, ep.a_cls[cls], cr, ub, resid, racc);
-                ep.s1[idx] = o.s_new; ep.g_hi[idx] = o.g_hi; ep.g_lo[idx] = o.g_lo;
+                ep.s1[idx] = o.s_new; emit_small(ep.g_hi, ep.g_lo, (int64_t)p * ep.ldN, row, o.g, ep.small_bf16 != 0);
             } else {
                 bool on = true;
                 if (ep.mask) on = (ep.mask[(int64_t)ep.slot_plan[p] * ep.mask_words + (row >> 5)] >> (row & 31)) & 1u;
@@ -520,9 +547,9 @@ __global__ void objective_reduce_kernel(const double* __restrict__ hinge, int gr
     if (threadIdx.x == 0) { double v = 0; for (int w = 0; w < (int)(blockDim.x >> 5); ++w) v += sh[w]; obj[p] = v; }
 }
 
-__global__ void split_tf32_kernel(const float* __restrict__ x, int64_t count, float* __restrict__ hi, float* __restrict__ lo) {
+__global__ void split_small_kernel(const float* __restrict__ x, int64_t count, int64_t ld, void* __restrict__ hi, void* __restrict__ lo, int bf16) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < count) { float h = tc::tf32_rn(x[i]); hi[i] = h; lo[i] = x[i] - h; }
+    if (i < count) emit_small(hi, lo, (i / ld) * ld, i % ld, x[i], bf16 != 0);
 }
 // out[p][j] = sum over the slots of j's m-tile of partial[slot][p][j % 128]   (test hook, fp64)
 __global__ void reduce_partial_kernel(const float* __restrict__ partial, const int32_t* __restrict__ mtile_slot_begin, int n_mma,
@@ -561,6 +588,20 @@ void launch_pack_tiles(const float* src, int64_t src_rows, int64_t src_cols, int
         const int64_t KB = cdiv(src_rows, kBlockK), RT = cdiv(src_cols, kTileM);
         pack_tiles_kernel<true><<<dim3((unsigned)KB, (unsigned)RT), 256, 0, s>>>(src, src_rows, src_cols, ld_src, dst, KB);
     }
+}
+void launch_pack_tiles_bf16(const float* src, int64_t src_rows, int64_t src_cols, int64_t ld_src, bool transpose, void* dst,
+                            cudaStream_t s) {
+    __nv_bfloat16* d = reinterpret_cast<__nv_bfloat16*>(dst);
+    if (!transpose) {
+        const int64_t KB = cdiv(src_cols, 64), RT = cdiv(src_rows, kTileM);
+        pack_tiles_bf16_kernel<false><<<dim3((unsigned)KB, (unsigned)RT), 256, 0, s>>>(src, src_rows, src_cols, ld_src, d, KB);
+    } else {
+        const int64_t KB = cdiv(src_rows, 64), RT = cdiv(src_cols, kTileM);
+        pack_tiles_bf16_kernel<true><<<dim3((unsigned)KB, (unsigned)RT), 256, 0, s>>>(src, src_rows, src_cols, ld_src, d, KB);
+    }
+}
+void launch_round_bf16(float* x, int64_t count, cudaStream_t s) {
+    round_bf16_kernel<<<(unsigned)cdiv(count, 256), 256, 0, s>>>(x, count);
 }
 void launch_scale_rows_to_f64(const float* phi, int64_t ld, int64_t row0, int64_t rows, int64_t n, const uint8_t* cls,
                               const double* a_cls, double* out, cudaStream_t s) {
@@ -608,7 +649,8 @@ static void launch_k2b_t(admm_handle* h, int Bact, bool resid, cudaStream_t s) {
     if (!attr_done) { cudaFuncSetAttribute(k2b_kernel<WJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_done = true; }
     dim3 grid((unsigned)cdiv(h->n, 16 * WJ), (unsigned)cdiv(Bact, K2_TP));
     k2b_kernel<WJ><<<grid, 256, smem, s>>>(h->d_Sinv, h->lds, h->d_rhs, h->d_s2, h->d_R, h->d_beta, h->n, h->ldn, Bact,
-                                               h->d_vhi, h->d_vlo, resid ? h->d_resid2 : nullptr);
+                                               h->d_vhi, h->d_vlo, h->opt.storage == ADMM_STORAGE_BF16 ? 1 : 0,
+                                               resid ? h->d_resid2 : nullptr);
 }
 void launch_k2b(admm_handle* h, int Bact, bool resid, cudaStream_t s) {
     switch (k2_wj(h)) {
@@ -642,13 +684,14 @@ void launch_convergence(admm_handle* h, int Bact, int grid1, int grid2, float to
                                                               h->d_res_slot);
     h->launch_count++;
 }
-void launch_make_t(admm_handle* h, int Bact, float* t_hi, float* t_lo, float* t_f32, cudaStream_t s) {
+void launch_make_t(admm_handle* h, int Bact, void* t_hi, void* t_lo, float* t_f32, cudaStream_t s) {
     dim3 grid((unsigned)cdiv(h->n, 128), Bact);
-    make_t_kernel<<<grid, 128, 0, s>>>(h->d_s2, h->d_R, h->d_beta, h->d_rho, h->n, h->ldn, Bact, t_hi, t_lo, t_f32);
+    make_t_kernel<<<grid, 128, 0, s>>>(h->d_s2, h->d_R, h->d_beta, h->d_rho, h->n, h->ldn, Bact, t_hi, t_lo, t_f32,
+                                       h->opt.storage == ADMM_STORAGE_BF16 ? 1 : 0);
     h->launch_count++;
 }
-void launch_split_tf32(const float* x, int64_t count, float* hi, float* lo, cudaStream_t s) {
-    split_tf32_kernel<<<(unsigned)cdiv(count, 256), 256, 0, s>>>(x, count, hi, lo);
+void launch_split_small(const float* x, int64_t count, int64_t ld, void* hi, void* lo, bool bf16, cudaStream_t s) {
+    split_small_kernel<<<(unsigned)cdiv(count, 256), 256, 0, s>>>(x, count, ld, hi, lo, bf16 ? 1 : 0);
 }
 void launch_reduce_partial(admm_handle* h, int nact, int n_mma, double* out, cudaStream_t s) {
     dim3 grid((unsigned)cdiv(h->n, 128), nact);

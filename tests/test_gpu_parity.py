@@ -154,6 +154,44 @@ def test_tf32_storage_parity_against_same_rounded_phi(b):
     assert ez.max() < 1e-2 and ey.max() < 1e-2 and et.max() < 1e-2
 
 
+def _round_bf16(x):
+    u = x.view(np.uint32).astype(np.uint64)
+    return (((u + 0x7FFF + ((u >> 16) & 1)) & 0xFFFF0000).astype(np.uint32)).view(np.float32)
+
+
+def test_bf16_storage_contractions(b):
+    """ADMM_STORAGE_BF16: the kernels consume Phi rounded to bf16 (exactly) and the plan operand as a bf16 hi/lo pair
+    (16 bits kept): against the fp64 product with the SAME rounded Phi the error is the 2^-17 of the pair."""
+    from workloads import make_workload
+    w = make_workload(0, n_target=333, n_lowdose=1001, n_iso=7)       # N = 1334, n = 168: ragged in both dims, 64-element k-blocks
+    Pr = _round_bf16(w.phi).astype(np.float64)
+    rng = np.random.default_rng(3)
+    h = b.admm_setup(w.phi, w.point_class, w.classes, storage=b.ADMM_STORAGE_BF16)
+    for which, Bp in ((1, 9), (0, 81), (1, 130), (0, 256)):
+        K = w.N if which == 0 else w.n
+        small = rng.standard_normal((Bp, K)).astype(np.float32)
+        got = b.admm_contract_probe(h, which, small)
+        exact = small.astype(np.float64) @ (Pr if which == 0 else Pr.T)
+        scale = np.abs(small.astype(np.float64)) @ (Pr if which == 0 else Pr.T)
+        assert np.max(np.abs(got - exact) / scale) < 2e-5, (which, Bp)
+    h.close()
+
+
+def test_bf16_storage_parity(b):
+    """Reading R18: against the oracle fed the SAME bf16-rounded Phi only the arithmetic differs (bf16 hi/lo plan operands,
+    undrained fp32 accumulation); against the original Phi it must stay inside north_star's 1e-2 bf16-storage budget."""
+    import copy
+    from workloads import default_rho, make_workload
+    w = make_workload(2, n_target=900, n_lowdose=1800, n_iso=9, grid=4)     # row masks, B = 16
+    rho = default_rho(w.beta)
+    wr = copy.copy(w); wr.phi = _round_bf16(w.phi)
+    ez, ey, et, eobj, _, _ = _parity(b, w, rho, 50, ref=_oracle(wr, rho, 50), storage=b.ADMM_STORAGE_BF16)
+    assert ez.max() < 1e-3 and ey.max() < 1e-3 and et.max() < 2e-3, (ez.max(), ey.max(), et.max())
+    ez, ey, et, eobj, _, _ = _parity(b, w, rho, 50, storage=b.ADMM_STORAGE_BF16)
+    assert ez.max() < 1e-2 and ey.max() < 1e-2 and et.max() < 1e-2, (ez.max(), ey.max(), et.max())
+    assert eobj.max() < 1e-2
+
+
 # ------------------------------------------------------------------------------------------ setup
 def test_preconditioner_matches_oracle(b):
     from oracle import admm

@@ -174,6 +174,8 @@ def main() -> None:
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (1 = the bench workload)")
     ap.add_argument("--ref-iters", type=int, default=40, help="oracle iterations per step for --impl reference / cpu_baseline")
+    ap.add_argument("--storage", default="fp32", choices=["fp32", "tf32", "bf16"],
+                    help="how Phi is stored / consumed (BASELINE.json config 4 variants); fp32 = 3xTF32, the 1e-4 path")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -204,7 +206,9 @@ def main() -> None:
     stream = torch.cuda.current_stream().cuda_stream
 
     phi_pinned = torch.from_numpy(w.phi).pin_memory()
-    h = b.admm_setup(phi_pinned, w.point_class, w.classes, device=local_rank, stream=stream)
+    storage = {"fp32": b.ADMM_STORAGE_FP32_3XTF32, "tf32": b.ADMM_STORAGE_FP32_TF32, "bf16": b.ADMM_STORAGE_BF16}[args.storage]
+    elem_bytes = 2 if args.storage == "bf16" else 4
+    h = b.admm_setup(phi_pinned, w.point_class, w.classes, device=local_rank, stream=stream, storage=storage)
     setup_t = b.admm_get_timing(h)
     mask_dev = None if w.row_mask is None else torch.from_numpy(w.row_mask.view(np.int32)).to(dev)
     outs = dict(t=torch.empty((w.B, w.n), dtype=torch.float32, device=dev),
@@ -252,7 +256,7 @@ def main() -> None:
         t0 = time.perf_counter()
         pi2 = 0
         for _ in range(n_e2e):
-            h2 = b.admm_setup(phi_pinned, w.point_class, w.classes, device=local_rank, stream=stream)
+            h2 = b.admm_setup(phi_pinned, w.point_class, w.classes, device=local_rank, stream=stream, storage=storage)
             host_out = b.admm_solve_batch(h2, weights, rho, w.row_mask, tol=TOL, max_iter=MAX_ITER)
             pi2 += b.admm_get_timing(h2)["plan_iters"]
             h2.close()
@@ -268,7 +272,7 @@ def main() -> None:
     # ---- roofline of the dominant kernel: CUDA events around every launch of a fixed-iteration solve
     roof = None
     if rank == 0:
-        hp = b.admm_setup(phi_pinned, w.point_class, w.classes, device=local_rank, stream=stream, profile_kernels=True)
+        hp = b.admm_setup(phi_pinned, w.point_class, w.classes, device=local_rank, stream=stream, profile_kernels=True, storage=storage)
         K_prof = 100
         b.admm_solve_batch(hp, weights, rho, mask_dev, fixed_iters=K_prof, out=outs)     # warm
         b.admm_solve_batch(hp, weights, rho, mask_dev, fixed_iters=K_prof, out=outs)
@@ -276,8 +280,9 @@ def main() -> None:
         hp.close()
         N, n, B = w.N, w.n, w.B
         # algorithmic bytes per launch: Phi once + state / operand traffic of that kernel
-        alg = {"k3_phi_v": 4.0 * N * n + 8.0 * n * B + 4.0 * N * B * 4,       # Phi, V hi/lo, s1 r+w, G hi+lo w
-               "k1_phiT_g": 4.0 * N * n + 8.0 * N * B + 4.0 * n * B}          # Phi^T, G hi/lo, W
+        eb = float(elem_bytes)
+        alg = {"k3_phi_v": eb * N * n + 2 * eb * n * B + 8.0 * N * B + 2 * eb * N * B,   # Phi, V hi/lo, s1 r+w, G hi+lo w
+               "k1_phiT_g": eb * N * n + 2 * eb * N * B + 4.0 * n * B}                   # Phi^T, G hi/lo, W
         dom = max(("k1_phiT_g", "k3_phi_v"), key=lambda k: kt[k]["total_ms"])
         avg_ms = kt[dom]["total_ms"] / max(kt[dom]["launches"], 1)
         peak, which = _peaks()
@@ -302,9 +307,11 @@ def main() -> None:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32 (3xTF32 tensor-core products, fp32 accumulate; S^-1 apply and block-2 state in f64)",
+            "dtype": {"fp32": "f32 (3xTF32 tensor-core products, fp32 accumulate; S^-1 apply and block-2 state in f64)",
+                      "tf32": "tf32-rounded Phi x tf32 hi/lo plan operands, fp32 accumulate; S^-1 apply in f64",
+                      "bf16": "bf16 Phi x bf16 hi/lo plan operands, fp32 accumulate; S^-1 apply in f64"}[args.storage],
             "data": "synthetic",
-            "config": {"workload": _workload_desc(w, args.config), "tol": TOL, "max_iter": MAX_ITER,
+            "config": {"workload": _workload_desc(w, args.config), "storage": args.storage, "tol": TOL, "max_iter": MAX_ITER,
                        "plans_per_gpu": w.B, "l2": "inputs larger than L2: Phi and Phi^T (2 x %.0f MB) are streamed every iteration" % (w.N * w.n * 4 / 1e6),
                        "parallelism": "plans sharded over ranks, Phi replicated" if world > 1 else "single GPU"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,

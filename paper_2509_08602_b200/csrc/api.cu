@@ -178,9 +178,10 @@ EpiParams base_epi(admm_handle* h) {
 int mma_passes(const admm_handle* h) { return h->opt.storage == ADMM_STORAGE_FP32_3XTF32 ? 3 : 2; }
 // fp32 path: drain the hi.hi TMEM accumulator every k-block (32 elements of K, 4 MMAs) -- see gemm_tc.cu
 int chunk_kb(const admm_handle* h) {
-    if (h->opt.storage != ADMM_STORAGE_FP32_3XTF32 || h->opt.kernel_path != ADMM_PATH_TCGEN05) return 0;
+    if (h->opt.kernel_path != ADMM_PATH_TCGEN05) return 0;
     if (h->opt.drain_kb < 0) return 0;
-    return h->opt.drain_kb > 0 ? h->opt.drain_kb : 1;
+    if (h->opt.drain_kb > 0) return h->opt.drain_kb;
+    return h->opt.storage == ADMM_STORAGE_BF16 ? 4 : 1;      // bf16 storage has a 1e-2 budget: drain less often
 }
 // plans per contraction pass
 int max_pass(const admm_handle* h) {

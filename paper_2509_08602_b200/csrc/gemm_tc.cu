@@ -487,9 +487,13 @@ __device__ __noinline__ void epilogue_unit_t(const TcLaunch& L, const TcUnit& un
                     Epi1Out o = epi1_element(so[j], q, a_k, cr[j], on ? ub[j] : 0.0f, RESID, racc);
                     const uint32_t off = (uint32_t)p * ldN;
                     s1p[off] = o.s_new;
-                    const float ghi = tc::tf32_rna(o.g);
-                    ghp[off] = ghi;
-                    glp[off] = tc::tf32_rna(o.g - ghi);
+                    if (ep.small_bf16) {
+                        emit_small(ep.g_hi, ep.g_lo, (int64_t)(ep.slot0 + p) * ep.ldN, row, o.g, true);
+                    } else {
+                        const float ghi = tc::tf32_rna(o.g);
+                        ghp[off] = ghi;
+                        glp[off] = tc::tf32_rna(o.g - ghi);
+                    }
                 } else {
                     hinge = on ? fmaxf(0.0f, sense * (thr - q)) : 0.0f;
                 }
@@ -609,7 +613,8 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
     const int chunk_kb = L.chunk_kb;
 
     if (threadIdx.x == 0) {
-        for (int i = 0; i < n_sa; ++i) { tc::mbar_init(&ctrl->sa_full[i], 1); tc::mbar_init(&ctrl->sa_empty[i], 4); }
+        // sa_empty: released by the 4 converter warps (3xTF32: the raw tile is in registers) or by the MMA commit (direct mode)
+        for (int i = 0; i < n_sa; ++i) { tc::mbar_init(&ctrl->sa_full[i], 1); tc::mbar_init(&ctrl->sa_empty[i], L.mma_passes == 3 ? 4 : 1); }
         for (int i = 0; i < n_sb; ++i) { tc::mbar_init(&ctrl->sb_full[i], 1); tc::mbar_init(&ctrl->sb_empty[i], 1); }
         for (int i = 0; i < 2; ++i) {
             tc::mbar_init(&ctrl->a_full[i], 4);
@@ -661,7 +666,7 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
                     if (++sa == n_sa) { sa = 0; pha ^= 1; }
                 }
                 if (ib.u < unit_end && tc::mbar_test_wait(&ctrl->sb_empty[sb], phb ^ 1)) {
-                    const int k0 = (L.units[ib.u].kb0 + ib.kb) * kBlockK;
+                    const int k0 = (L.units[ib.u].kb0 + ib.kb) * L.kblk;
                     tc::mbar_arrive_expect_tx(&ctrl->sb_full[sb], bbytes);
                     tc::tma_load_2d(b_ring + sb * bbytes, &L.map_small_hi, &ctrl->sb_full[sb], k0, 0, tc::kEvictLast);
                     tc::tma_load_2d(b_ring + sb * bbytes + bbytes / 2, &L.map_small_lo, &ctrl->sb_full[sb], k0, 0, tc::kEvictLast);
@@ -672,8 +677,12 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
         }
     } else if (warp == 1) {
         // ------------------------------------------------------------ UMMA issuer (warp-uniform loop, one elected lane issues)
-        const uint32_t idesc_wide = tc::umma_idesc(2u, kTileM, (uint32_t)(2 * n_mma));
-        const uint32_t idesc_one = tc::umma_idesc(2u, kTileM, (uint32_t)n_mma);
+        const bool direct = L.mma_passes != 3;     // Phi already exact in the operand format (tf32 / bf16 storage): A straight from smem
+        const uint32_t fmt = L.mma_kind == 1 ? 1u : 2u;
+        const uint32_t idesc_wide = tc::umma_idesc(fmt, kTileM, (uint32_t)(2 * n_mma));
+        const uint32_t idesc_one = tc::umma_idesc(fmt, kTileM, (uint32_t)n_mma);
+        const uint64_t a_desc0 = tc::umma_desc_k_sw128(tc::smem_u32(a_ring));
+        int sa = 0; uint32_t pha = 0;              // smem A ring (direct mode)
         const uint64_t b_desc0 = tc::umma_desc_k_sw128(tc::smem_u32(b_ring));
         const uint64_t b_step = (uint64_t)(bbytes >> 4);
         uint64_t b_desc = b_desc0;
@@ -690,6 +699,24 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
                 const uint32_t d_small = d_main + n_mma;
                 for (int kb = 0; kb < nkb; ++kb) {
                     tc::mbar_wait(&ctrl->sb_full[sb], phb);     // the small operand landed (async proxy)
+                    if (direct) {
+                        tc::mbar_wait(&ctrl->sa_full[sa], pha); // the big operand's tile landed (async proxy): it IS the A operand
+                        tc::tcgen05_fence_after();
+                        const uint64_t a_desc = a_desc0 + (uint64_t)(sa * (kTileBytes >> 4));
+                        if (tc::elect_one()) {
+                            // one MMA per 32-byte k-step (8 tf32 / 16 bf16 elements): D[:, 0:2n) += A . [B_hi ; B_lo]^T
+#pragma unroll
+                            for (int k = 0; k < 4; ++k) {
+                                if (fmt == 1u) tc::umma_f16(d_main, a_desc + 2 * k, b_desc + 2 * k, idesc_wide, 1u);
+                                else tc::umma_tf32(d_main, a_desc + 2 * k, b_desc + 2 * k, idesc_wide, 1u);
+                            }
+                            tc::umma_commit(&ctrl->sb_empty[sb]);
+                            tc::umma_commit(&ctrl->sa_empty[sa]);
+                            if (kb == nkb - 1) tc::umma_commit(&ctrl->d_full[a]);
+                        }
+                        __syncwarp();
+                        if (++sa == n_sa) { sa = 0; pha ^= 1; }
+                    } else {
                     tc::mbar_wait(&ctrl->a_full[t], tph);       // the converter's hi/lo are in TMEM
                     tc::tcgen05_fence_after();
                     const uint32_t a_hi = tmem_base + kAcol + t * 64;
@@ -704,6 +731,7 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
                         if (kb == nkb - 1) tc::umma_commit(&ctrl->d_full[a]);
                     }
                     __syncwarp();
+                    }
                     b_desc += b_step;
                     if (++sb == n_sb) { sb = 0; phb ^= 1; b_desc = b_desc0; }
                     if (++t == 2) { t = 0; tph ^= 1; }
@@ -712,6 +740,7 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
             }
         }
     } else if (warp >= kConvWarp0 && warp < kDrainWarp0) {
+        if (L.mma_passes == 3) {
         // ------------------------------------------------------------ converter: smem fp32 row -> TMEM hi | lo
         // hi = tf32_rna(x) (round to nearest: lo = x - hi is then symmetric in sign, so the tensor core's truncation of
         // lo's low bits is unbiased; with a truncated hi, lo >= 0 for Phi >= 0 and the products came out 2^-22 too small)
@@ -756,6 +785,7 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
                 if (++sa == n_sa) { sa = 0; pha ^= 1; }
                 if (++t == 2) { t = 0; tph ^= 1; }
             }
+        }
         }
     } else if (warp >= kDrainWarp0 && warp < kEpiWarp0) {
         // ------------------------------------------------------------ drain (row = TMEM lane): TMEM -> fp32 master sums -> qs
@@ -923,7 +953,8 @@ admm_status tc_launch(admm_handle* h, const TcLaunch& L) {
         h->err = "tc_launch: fewer than 2 pipeline stages fit in shared memory";
         return ADMM_EINVAL;
     }
-    if (L.mma_passes == 3) {
+    if (L.mma_passes == 3 || n_mma <= kF32MaxMmaN) {
+        // the staged kernel: 3xTF32 (converter + TS MMAs), or "direct" for tf32 / bf16 storage (A from shared memory)
         if (n_mma > kF32MaxMmaN) { h->err = "tc_launch: the fp32 path needs n_mma <= 96"; return ADMM_EINVAL; }
         if (f32_a_stages(n_mma) < 2) { h->err = "tc_launch: fewer than 2 pipeline stages fit in shared memory"; return ADMM_EINVAL; }
         TcLaunch L2 = L;

@@ -54,7 +54,8 @@ enum {
     ADMM_STORAGE_FP32_3XTF32 = 0, /* fp32 storage, hi/lo split on chip, 3 tf32 MMAs: the fp32 path (1e-4 parity) */
     ADMM_STORAGE_FP32_TF32   = 1, /* Phi rounded once to tf32 (kept in an fp32 container), 2 tf32 MMAs */
     ADMM_STORAGE_BF16        = 2, /* Phi rounded once to bf16 (half the HBM bytes), plan operands as bf16 hi/lo pairs, 2 bf16 MMAs (1e-2 parity) */
-    ADMM_STORAGE_CSR         = 3  /* thresholded CSR                                     [not built yet] */
+    ADMM_STORAGE_CSR         = 3  /* entries below csr_rel_threshold * max|Phi| dropped, CSR of Phi and of Phi^T, SpMM on the FP32 ALUs
+                                     (kernel_path is ignored); S is formed from the thresholded matrix */
 };
 
 /* Which kernels run the two Phi contractions. */
@@ -71,7 +72,7 @@ typedef struct {
     int32_t check_every;       /* stopping rule tested every this many iterations; 0 => 10          */
     float   eps_abs;           /* absolute part of the stopping rule; 0 => 1e-6 (reading R7) */
     int32_t compaction;        /* 1: converged plans are swapped out of the active batch; 0: masked only */
-    float   csr_rel_threshold; /* ADMM_STORAGE_CSR only                                             */
+    float   csr_rel_threshold; /* ADMM_STORAGE_CSR only; 0 => 1e-3                                  */
     int32_t profile_kernels;   /* 1: CUDA events around every hot-path kernel (admm_get_kernel_times) */
     int32_t drain_kb;          /* fp32 path: the TMEM accumulator is drained into fp32 registers every this many
                                   32-element k-blocks; 0 => default, -1 => never            */
@@ -149,7 +150,7 @@ admm_status admm_get_preconditioner(admm_handle* h, double* D, double* R, double
  * Wall/device times of the last calls, milliseconds:
  *   ms[0] upload+transpose  ms[1] S = I + A^A^^T (syrk)  ms[2] Cholesky + inverse  ms[3] setup total
  *   ms[4] last solve: iterations (device)   ms[5] last solve: finalise (device)   ms[6] last solve total (host wall)
- *   ms[7] reserved
+ *   ms[7] ADMM_STORAGE_CSR: density nnz / (N n) of the thresholded Phi, else 0
  *   plan_iters = sum over plans of iterations done in the last solve.
  */
 admm_status admm_get_timing(admm_handle* h, double ms[8], int64_t* plan_iters);

@@ -119,7 +119,8 @@ def admm_default_options() -> admm_options:
 def admm_setup(phi, point_class, classes: Sequence, *, storage: int = ADMM_STORAGE_FP32_3XTF32,
                kernel_path: int = ADMM_PATH_TCGEN05, device: int = 0, stream: Optional[int] = None,
                check_every: int = 10, eps_abs: float = 1e-6, compaction: bool = True,
-               profile_kernels: bool = False, drain_kb: int = 0, k1_slab_kb: int = 0) -> Handle:
+               profile_kernels: bool = False, drain_kb: int = 0, k1_slab_kb: int = 0,
+               csr_rel_threshold: float = 0.0) -> Handle:
     """phi: [N, n] float32, numpy (host) or torch CUDA tensor, row-major (last stride 1).
     classes: sequence of objects with .sense, .threshold, .hard (e.g. workloads.ClassSpec)."""
     if _is_torch(phi):
@@ -138,6 +139,7 @@ def admm_setup(phi, point_class, classes: Sequence, *, storage: int = ADMM_STORA
     o.check_every, o.eps_abs, o.compaction, o.profile_kernels = check_every, eps_abs, int(compaction), int(profile_kernels)
     o.drain_kb = int(drain_kb)
     o.k1_slab_kb = int(k1_slab_kb)
+    o.csr_rel_threshold = float(csr_rel_threshold)
     out = C.c_void_p()
     st = _lib.admm_setup(C.byref(out), _ptr(phi), on_device, N, n, ld, _ptr(pc), cls, len(classes), C.byref(o))
     _check(st, None)
@@ -193,7 +195,7 @@ def admm_get_preconditioner(h: Handle, want_sinv: bool = True):
 def admm_get_timing(h: Handle) -> dict:
     ms = (C.c_double * 8)(); it = C.c_int64()
     _check(_lib.admm_get_timing(h.ptr, C.byref(ms), C.byref(it)), h.ptr)
-    keys = ["upload_ms", "syrk_ms", "factor_ms", "setup_ms", "iterate_ms", "finalise_ms", "solve_wall_ms", "reserved"]
+    keys = ["upload_ms", "syrk_ms", "factor_ms", "setup_ms", "iterate_ms", "finalise_ms", "solve_wall_ms", "csr_density"]
     d = {k: ms[i] for i, k in enumerate(keys)}
     d["plan_iters"] = it.value
     return d

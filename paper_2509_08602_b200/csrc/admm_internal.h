@@ -96,6 +96,10 @@ struct admm_handle {
     float* d_phiT = nullptr;       // [n][ldN] row-major (SIMT cross-check path only)
     float* d_phi_t = nullptr;      // tile-major Phi:   [ceil(N/128)][ceil(n/32)][128][32]  (K3 / objective big operand)
     float* d_phiT_t = nullptr;     // tile-major Phi^T: [ceil(n/128)][ceil(N/32)][128][32]  (K1 big operand)
+    // ADMM_STORAGE_CSR: thresholded Phi as CSR (rows = points) and the CSR of Phi^T (rows = time variables)
+    int64_t *d_csr_ptr = nullptr, *d_csrT_ptr = nullptr; int32_t *d_csr_col = nullptr, *d_csrT_col = nullptr;
+    float *d_csr_val = nullptr, *d_csrT_val = nullptr; int64_t csr_nnz = 0; float csr_tau = 0.f;
+    float* d_small_t = nullptr;    // [max(N, n)][<= 256] element-major copy of the plan operand of one SpMM
     uint8_t* d_point_class = nullptr;
     double* d_R = nullptr;         // [n]
     double* d_Sinv = nullptr;      // [n][lds], lds = n rounded up to even (16-byte rows for cp.async), pad = 0
@@ -142,6 +146,12 @@ admm_status tc_init(admm_handle* h);                       // resolves cuTensorM
 admm_status tc_make_map(admm_handle* h, CUtensorMap* out, const void* base, int64_t rows, int64_t cols,
                         int64_t ld_elems, int box_rows, int elem_bytes = 4);
 admm_status tc_launch(admm_handle* h, const TcLaunch& L);
+
+// ---- csr.cu
+admm_status csr_threshold(admm_handle* h);
+admm_status csr_build(admm_handle* h);
+void launch_csr_k1(admm_handle* h, int slot0, int nact, int n_mma, cudaStream_t s);
+void launch_csr_k3(admm_handle* h, int nact, const float* vhi, const float* vlo, float* qbuf, cudaStream_t s);
 
 // ---- kernels.cu  (everything that is not a tcgen05 contraction)
 void launch_pack_tiles(const float* src, int64_t src_rows, int64_t src_cols, int64_t ld_src, bool transpose, float* dst, cudaStream_t s);

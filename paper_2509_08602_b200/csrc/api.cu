@@ -146,7 +146,7 @@ struct Profiler {
 };
 
 void free_all(admm_handle* h) {
-    void* ptrs[] = {h->d_phi, h->d_phiT, h->d_phi_t, h->d_phiT_t, h->d_point_class, h->d_R, h->d_Sinv, h->d_s1, h->d_ghi, h->d_glo, h->d_s2, h->d_rhs,
+    void* ptrs[] = {h->d_phi, h->d_phiT, h->d_phi_t, h->d_phiT_t, h->d_csr_ptr, h->d_csrT_ptr, h->d_csr_col, h->d_csrT_col, h->d_csr_val, h->d_csrT_val, h->d_small_t, h->d_point_class, h->d_R, h->d_Sinv, h->d_s1, h->d_ghi, h->d_glo, h->d_s2, h->d_rhs,
                     h->d_vhi, h->d_vlo, h->d_partial, h->d_resid1, h->d_resid2, h->d_hinge, h->d_mask, h->d_slot_plan,
                     h->d_utab, h->d_crtab, h->d_beta, h->d_rho, h->d_active_counts, h->d_conv_flags, h->d_res_slot,
                     h->d_rowtmp, h->d_rowtmp2, h->d_units_k1, h->d_cta_begin_k1, h->d_mtile_slot_begin, h->d_units_k3,
@@ -288,6 +288,7 @@ static admm_status setup_impl(admm_handle* h, const float* phi, int32_t phi_on_d
     CU_TRY(h, cudaMemcpy2DAsync(h->d_phi, (size_t)h->ldn * 4, phi, (size_t)ld * 4, (size_t)n * 4, (size_t)N,
                                 phi_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
     CU_TRY(h, cudaMemcpyAsync(h->d_point_class, point_class, (size_t)N, cudaMemcpyHostToDevice, st));
+    if (h->opt.storage == ADMM_STORAGE_CSR) ST_TRY(csr_threshold(h));
     // reduced storage: Phi is rounded ONCE here, so S below is formed from the matrix the kernels consume (SURVEY H-c)
     if (h->opt.storage == ADMM_STORAGE_FP32_TF32) launch_round_tf32(h->d_phi, N * h->ldn, st);
     if (bf16) launch_round_bf16(h->d_phi, N * h->ldn, st);
@@ -337,6 +338,13 @@ static admm_status setup_impl(admm_handle* h, const float* phi, int32_t phi_on_d
     launch_finish_S(h->d_Sinv, n, h->d_R, st);
     if (cudaStreamSynchronize(st) != cudaSuccess) { cleanup(); h->err = "S formation failed"; return ADMM_ECUDA; }
     if (tc_path) { cudaFree(h->d_phi); h->d_phi = nullptr; }      // only the tile-major copies stay resident
+    if (h->opt.storage == ADMM_STORAGE_CSR) {
+        ST_TRY(csr_build(h));
+        if (cudaStreamSynchronize(st) != cudaSuccess) { cleanup(); h->err = "CSR build failed"; return ADMM_ECUDA; }
+        cudaFree(h->d_phi); h->d_phi = nullptr; cudaFree(h->d_phiT); h->d_phiT = nullptr;
+        ST_TRY(dev_alloc(h, &h->d_small_t, std::max(N, n) * (int64_t)kMaxMmaN));
+        h->ms[7] = (double)h->csr_nnz / ((double)N * (double)n);
+    }
     const double t2 = now_ms();
 
     // ---- S2: Cholesky + explicit inverse in fp64, shared by every plan and every rho (:222)
@@ -393,7 +401,8 @@ static admm_status setup_impl(admm_handle* h, const float* phi, int32_t phi_on_d
         h->slots_k1 = msb.back();
     } else {
         const int m_tiles = (int)cdiv(n, kTileM);
-        const int splits = (int)std::max<int64_t>(1, std::min<int64_t>(64, (2 * h->sm_count) / std::max<int64_t>(1, cdiv(n, 64))));
+        const int splits = h->opt.storage == ADMM_STORAGE_CSR ? 1 :
+                           (int)std::max<int64_t>(1, std::min<int64_t>(64, (2 * h->sm_count) / std::max<int64_t>(1, cdiv(n, 64))));
         msb.resize(m_tiles + 1);
         for (int i = 0; i <= m_tiles; ++i) msb[i] = i * splits;
         h->slots_k1 = m_tiles * splits; h->grid_k1 = splits;     // grid_k1 carries the split count on the SIMT path
@@ -427,8 +436,12 @@ admm_status admm_setup(admm_handle** out, const float* phi, int32_t phi_on_devic
     if (opt) o = *opt; else admm_default_options(&o);
     if (o.check_every <= 0) o.check_every = 10;
     if (!(o.eps_abs > 0.f)) o.eps_abs = 1e-6f;
-    if (o.storage != ADMM_STORAGE_FP32_3XTF32 && o.storage != ADMM_STORAGE_FP32_TF32 && o.storage != ADMM_STORAGE_BF16) {
-        g_setup_err = "storage mode not built yet (FP32_3XTF32, FP32_TF32 and BF16 are)"; return ADMM_EINVAL;
+    if (o.storage < ADMM_STORAGE_FP32_3XTF32 || o.storage > ADMM_STORAGE_CSR) { g_setup_err = "unknown storage mode"; return ADMM_EINVAL; }
+    if (o.storage == ADMM_STORAGE_CSR) {
+        // sparse contractions run on the plain FP32 ALUs with the orchestration of the cross-check path
+        o.kernel_path = ADMM_PATH_SIMT;
+        if (!(o.csr_rel_threshold > 0.f)) o.csr_rel_threshold = 1e-3f;
+        if (!(o.csr_rel_threshold < 1.f)) { g_setup_err = "csr_rel_threshold must be in (0, 1)"; return ADMM_EINVAL; }
     }
     if (o.storage == ADMM_STORAGE_BF16 && o.kernel_path != ADMM_PATH_TCGEN05) {
         g_setup_err = "ADMM_STORAGE_BF16 exists on the tcgen05 path only"; return ADMM_EINVAL;

@@ -661,6 +661,7 @@ void launch_k2b(admm_handle* h, int Bact, bool resid, cudaStream_t s) {
     h->launch_count++;
 }
 void launch_simt_k1(admm_handle* h, int slot0, int nact, int n_mma, int splits, cudaStream_t s) {
+    if (h->opt.storage == ADMM_STORAGE_CSR) { launch_csr_k1(h, slot0, nact, n_mma, s); return; }
     const int64_t k_per_split = cdiv(cdiv(h->N, splits), 16) * 16;
     dim3 grid((unsigned)cdiv(h->n, 64), (unsigned)cdiv(nact, 64), splits);
     simt_contract_kernel<EPI_K1_PARTIAL><<<grid, 256, 0, s>>>(h->d_phiT, h->n, h->ldN, h->d_ghi + (int64_t)slot0 * h->ldN,
@@ -672,6 +673,12 @@ void launch_simt_k3(admm_handle* h, const EpiParams& ep, int epi, const float* v
                     cudaStream_t s) {
     // vhi / vlo point at the first slot of this pass
     const int nact = ep.n_slots_active;
+    if (h->opt.storage == ADMM_STORAGE_CSR) {
+        launch_csr_k3(h, nact, vhi, vlo, qbuf, s);
+        simt_epilogue_kernel<<<(unsigned)cdiv(h->N, 128), 128, 0, s>>>(ep, epi, qbuf);
+        h->launch_count += 1;
+        return;
+    }
     dim3 grid((unsigned)cdiv(h->N, 64), (unsigned)cdiv(nact, 64), 1);
     simt_contract_kernel<EPI_K3_STATE><<<grid, 256, 0, s>>>(h->d_phi, h->N, h->ldn, vhi, vlo, nact, h->ldn, h->n, h->n,
                                                              qbuf, h->ldN, 0, 1);

@@ -192,6 +192,35 @@ def test_bf16_storage_parity(b):
     assert eobj.max() < 1e-2
 
 
+def test_csr_storage_parity_against_thresholded_phi(b):
+    """ADMM_STORAGE_CSR (config 4's sparse variant): entries below 1e-3 max(Phi) are dropped; the oracle is run on the
+    SAME thresholded matrix, so the fp32 path's 1e-4 applies; the density is reported through admm_get_timing."""
+    import copy
+    from workloads import default_rho, make_workload
+    w = make_workload(2, n_target=1100, n_lowdose=2300, n_iso=18, grid=4)       # 9 targets: a point sees mostly its own isocenters
+    rho = default_rho(w.beta)
+    wt = copy.copy(w); wt.phi = np.where(w.phi < np.float32(1e-3) * w.phi.max(), np.float32(0), w.phi)
+    density = np.count_nonzero(wt.phi) / wt.phi.size
+    assert 0.02 < density < 0.9
+    ref = _oracle(wt, rho, 50)
+    h = b.admm_setup(w.phi, w.point_class, w.classes, storage=b.ADMM_STORAGE_CSR, csr_rel_threshold=1e-3)
+    assert abs(b.admm_get_timing(h)["csr_density"] - density) < 1e-9
+    out = b.admm_solve_batch(h, w.weights, rho, w.row_mask, fixed_iters=50)
+    ez, ey = stacked_errors(_gpu_states(b, h, w.B), ref)
+    et = t_errors(out["t"], ref["t"])
+    assert ez.max() < TOL_FP32 and ey.max() < TOL_FP32 and et.max() < TOL_FP32, (ez.max(), ey.max(), et.max())
+    # the two SpMMs alone, against the fp64 product with the thresholded matrix
+    P = wt.phi.astype(np.float64)
+    rng = np.random.default_rng(7)
+    for which, Bp in ((0, 40), (1, 81)):
+        small = rng.standard_normal((Bp, w.N if which == 0 else w.n)).astype(np.float32)
+        got = b.admm_contract_probe(h, which, small)
+        exact = small.astype(np.float64) @ (P if which == 0 else P.T)
+        scale = np.abs(small.astype(np.float64)) @ (P if which == 0 else P.T) + 1e-30
+        assert np.max(np.abs(got - exact) / scale) < 2e-6, which
+    h.close()
+
+
 # ------------------------------------------------------------------------------------------ setup
 def test_preconditioner_matches_oracle(b):
     from oracle import admm

@@ -46,7 +46,10 @@ def test_no_cpu_fallback_and_argument_errors(binding):
         assert e.value.status == binding.ADMM_ECUDA and "no CPU fallback" in str(e.value)
     # argument validation happens before any device work
     with pytest.raises(binding.AdmmError) as e:
-        binding.admm_setup(w.phi, w.point_class, w.classes, storage=binding.ADMM_STORAGE_CSR)
+        binding.admm_setup(w.phi, w.point_class, w.classes, storage=7)                      # unknown storage mode
+    assert e.value.status == binding.ADMM_EINVAL
+    with pytest.raises(binding.AdmmError) as e:
+        binding.admm_setup(w.phi, w.point_class, w.classes, storage=binding.ADMM_STORAGE_BF16, kernel_path=binding.ADMM_PATH_SIMT)
     assert e.value.status == binding.ADMM_EINVAL
     bad = [type("C", (), dict(sense=2, threshold=1.0, hard=0))(), w.classes[1]]
     with pytest.raises(binding.AdmmError) as e:

@@ -401,7 +401,7 @@ static admm_status setup_impl(admm_handle* h, const float* phi, int32_t phi_on_d
         h->slots_k1 = msb.back();
     } else {
         const int m_tiles = (int)cdiv(n, kTileM);
-        const int splits = h->opt.storage == ADMM_STORAGE_CSR ? 1 :
+        const int splits = h->opt.storage == ADMM_STORAGE_CSR ? (int)std::max<int64_t>(1, std::min<int64_t>(32, N / 8192)) :
                            (int)std::max<int64_t>(1, std::min<int64_t>(64, (2 * h->sm_count) / std::max<int64_t>(1, cdiv(n, 64))));
         msb.resize(m_tiles + 1);
         for (int i = 0; i <= m_tiles; ++i) msb[i] = i * splits;

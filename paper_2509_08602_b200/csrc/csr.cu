@@ -75,11 +75,12 @@ __global__ void transpose_sum_kernel(const float* __restrict__ hi, const float* 
 // w, w+4, ..; lanes = plans.  The non-zeros of a row are read 32 at a time (coalesced) and broadcast by shuffles.
 // Results go through shared memory so the stores are coalesced along the rows.
 //   K1_LAYOUT = false: out[q * out_ld + m]                                  (Q buffer [plan][point])
-//   K1_LAYOUT = true : out[((m / 128) * n_mma + q) * 128 + m % 128]          (the partial-sum layout K2a reads, one slot per m-tile)
+//   K1_LAYOUT = true : out[(((m / 128) * splits + blockIdx.y) * n_mma + q) * 128 + m % 128]   (the partial-sum layout K2a reads;
+//                      the rows of Phi^T are long, N * density non-zeros, so each is cut into `splits` segments = slots)
 template <bool K1_LAYOUT>
 __global__ void __launch_bounds__(128) csr_spmm_kernel(const int64_t* __restrict__ ptr, const int32_t* __restrict__ col,
                                                        const float* __restrict__ val, int64_t M, const float* __restrict__ Yt,
-                                                       int ldq, int nq, float* __restrict__ out, int64_t out_ld, int n_mma) {
+                                                       int ldq, int nq, float* __restrict__ out, int64_t out_ld, int n_mma, int splits) {
     extern __shared__ float tile[];                       // [ldq][33]
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int qc = ldq >> 5;                              // <= 8
@@ -88,7 +89,8 @@ __global__ void __launch_bounds__(128) csr_spmm_kernel(const int64_t* __restrict
         const int64_t m = m0 + rr;
         float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         if (m < M) {
-            const int64_t kb = ptr[m], ke = ptr[m + 1];
+            const int64_t r0 = ptr[m], len = ptr[m + 1] - r0;
+            const int64_t kb = r0 + len * blockIdx.y / splits, ke = r0 + len * (blockIdx.y + 1) / splits;
             for (int64_t k0 = kb; k0 < ke; k0 += 32) {
                 const int cnt = (int)min((int64_t)32, ke - k0);
                 const int myc = lane < cnt ? col[k0 + lane] : 0;
@@ -112,7 +114,7 @@ __global__ void __launch_bounds__(128) csr_spmm_kernel(const int64_t* __restrict
     for (int q = warp; q < nq; q += 4) {
         if (m >= M) continue;
         const float v = tile[q * 33 + lane];
-        if (K1_LAYOUT) out[((m / kTileM) * n_mma + q) * kTileM + (m % kTileM)] = v;
+        if (K1_LAYOUT) out[(((m / kTileM) * splits + blockIdx.y) * n_mma + q) * kTileM + (m % kTileM)] = v;
         else out[(int64_t)q * out_ld + m] = v;
     }
 }
@@ -182,8 +184,9 @@ void launch_csr_k1(admm_handle* h, int slot0, int nact, int n_mma, cudaStream_t 
     const float* hi = reinterpret_cast<const float*>(h->d_ghi) + (int64_t)slot0 * h->ldN;
     const float* lo = reinterpret_cast<const float*>(h->d_glo) + (int64_t)slot0 * h->ldN;
     transpose_sum_kernel<<<dim3((unsigned)cdiv(h->N, 32), (unsigned)(ldq / 32)), dim3(32, 8), 0, s>>>(hi, lo, nact, h->N, h->ldN, h->d_small_t, ldq);
-    csr_spmm_kernel<true><<<(unsigned)cdiv(h->n, 32), 128, (size_t)ldq * 33 * 4, s>>>(h->d_csrT_ptr, h->d_csrT_col, h->d_csrT_val, h->n,
-                                                                                      h->d_small_t, ldq, nact, h->d_partial, 0, n_mma);
+    const int splits = h->grid_k1;          // partial-sum slots per m-tile (api.cu)
+    csr_spmm_kernel<true><<<dim3((unsigned)cdiv(h->n, 32), (unsigned)splits), 128, (size_t)ldq * 33 * 4, s>>>(
+        h->d_csrT_ptr, h->d_csrT_col, h->d_csrT_val, h->n, h->d_small_t, ldq, nact, h->d_partial, 0, n_mma, splits);
     h->launch_count += 2;
 }
 // qbuf[plan][point] = Phi . V for the nact plans whose operand starts at vhi / vlo
@@ -191,6 +194,6 @@ void launch_csr_k3(admm_handle* h, int nact, const float* vhi, const float* vlo,
     const int ldq = (int)cdiv(nact, 32) * 32;
     transpose_sum_kernel<<<dim3((unsigned)cdiv(h->n, 32), (unsigned)(ldq / 32)), dim3(32, 8), 0, s>>>(vhi, vlo, nact, h->n, h->ldn, h->d_small_t, ldq);
     csr_spmm_kernel<false><<<(unsigned)cdiv(h->N, 32), 128, (size_t)ldq * 33 * 4, s>>>(h->d_csr_ptr, h->d_csr_col, h->d_csr_val, h->N,
-                                                                                       h->d_small_t, ldq, nact, qbuf, h->ldN, 0);
+                                                                                       h->d_small_t, ldq, nact, qbuf, h->ldN, 0, 1);
     h->launch_count += 2;
 }

@@ -130,6 +130,52 @@ def test_fixed_k_parity_more_than_one_pass_of_plans(b):
     assert ez.max() < TOL_FP32 and ey.max() < TOL_FP32 and et.max() < TOL_FP32
 
 
+def test_fixed_k_parity_config1_full_size(b):
+    """BASELINE.json configs[1] at full size (N = 60000, n = 1440, B = 81), the launch configuration bench.py times:
+    every plan's K = 50 iterate against the fp64 oracle, element by element (north_star: 1e-4 on the fp32 path)."""
+    from workloads import make_workload, scaled_rho
+    w = make_workload(1)
+    rho = scaled_rho(w.beta, w.point_class)
+    ez, ey, et, eobj, out, _ = _parity(b, w, rho, 50)
+    assert ez.max() < TOL_FP32 and ey.max() < TOL_FP32 and et.max() < TOL_FP32, (ez.max(), ey.max(), et.max())
+    assert eobj.max() < 1e-4
+
+
+@pytest.mark.skipif(os.environ.get("ADMM_BIG_TESTS") != "1", reason="full-size config 2 (17 GB Phi, ~3 min): set ADMM_BIG_TESTS=1")
+def test_config2_full_size_sampled_outputs(b):
+    """BASELINE.json configs[2] at full size (N = 450000, n = 9600): the oracle cannot run there in test time, so the two
+    contractions are checked on SAMPLED outputs the fp64 definition gives one by one (rows / columns of Phi drawn at random,
+    including the ragged last tile), and the iteration on properties that hold at any size: plan p in the batch equals
+    the same plan run alone (bit-exact), and the residual norms returned equal those recomputed from the read-back state."""
+    import torch
+    from workloads import make_workload, scaled_rho
+    w = make_workload(2)
+    rng = np.random.default_rng(11)
+    h = b.admm_setup(torch.from_numpy(w.phi), w.point_class, w.classes)
+    for which in (0, 1):
+        K = w.N if which == 0 else w.n
+        rows = w.n if which == 0 else w.N
+        small = rng.standard_normal((24, K)).astype(np.float32)
+        got = b.admm_contract_probe(h, which, small)
+        idx = np.unique(np.concatenate([rng.integers(0, rows, 200), [0, rows - 1, rows - 2]]))
+        sub = (w.phi[:, idx] if which == 0 else w.phi[idx, :].T).astype(np.float64)          # [K, samples]
+        exact = small.astype(np.float64) @ sub
+        scale = np.abs(small.astype(np.float64)) @ sub
+        assert np.max(np.abs(got[:, idx] - exact) / scale) < 1e-6, which
+    rho = scaled_rho(w.beta, w.point_class)
+    mask = torch.from_numpy(w.row_mask.view(np.int32)).cuda()
+    out = b.admm_solve_batch(h, w.weights, rho, mask, fixed_iters=12)
+    p = 40
+    st_batch = b.admm_get_state(h, p)
+    one = w.subset([p])
+    o1 = b.admm_solve_batch(h, one.weights, rho[[p]], one.row_mask, fixed_iters=12)
+    st_one = b.admm_get_state(h, 0)
+    for a, c in zip(st_batch, st_one):
+        assert np.array_equal(a, c)
+    assert np.array_equal(o1["t"][0], out["t"][p])
+    h.close()
+
+
 def test_simt_cross_check_path(b):
     from workloads import default_rho, make_workload
     w = make_workload(0, n_target=500, n_lowdose=900, n_iso=5)

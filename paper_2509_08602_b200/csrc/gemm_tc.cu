@@ -55,57 +55,62 @@ struct EpiCtx {
 };
 
 // 16 consecutive columns c0..c0+15 of this thread's row: q[jj] = accumulator of plan (slot0 + c0 + jj).
-// Deliberately NOT inlined and with a rolled column loop (q, so, mw live in local memory): unrolled it is ~6000
-// instructions per call site and the unit epilogue then runs at instruction-cache-miss speed (ncu: stall_no_inst).
-__device__ __noinline__ void epi_cols16(const TcLaunch& L, const EpiCtx& cx, int c0, const float* q) {
+// Inlined, arrays in registers, the 16 state loads of the group in flight together (unconditional, indices clamped; only
+// the stores are predicated) -- see epilogue_unit_t for why.
+__device__ __forceinline__ void epi_cols16(const TcLaunch& L, const EpiCtx& cx, int c0, const float (&q)[16]) {
     const EpiParams& ep = L.ep;
     const int n_act = ep.n_slots_active;
     const int epi = L.epi;
     if (epi == EPI_K1_PARTIAL) {
         float* dst = ep.partial + ((int64_t)cx.slot * ep.n_mma) * kTileM + cx.lrow;
-#pragma unroll 4
+#pragma unroll
         for (int jj = 0; jj < 16; ++jj)
             if (c0 + jj < n_act) dst[(int64_t)(c0 + jj) * kTileM] = q[jj];
         return;
     }
     if (epi == EPI_RAW) {
-#pragma unroll 4
+#pragma unroll
         for (int jj = 0; jj < 16; ++jj)
             if (c0 + jj < n_act && cx.valid) ep.qraw[(int64_t)(ep.slot0 + c0 + jj) * ep.ldN + cx.row] = q[jj];
         return;
     }
+    if (c0 >= n_act) return;                                         // warp-uniform
+    const int p_last = n_act - 1;
+    const bool has_mask = ep.mask != nullptr;
+    const uint32_t* mrow = has_mask ? ep.mask + cx.mword : reinterpret_cast<const uint32_t*>(ep.slot_plan);
+    const float* s1c = ep.s1 + (int64_t)ep.slot0 * ep.ldN + cx.row;     // cx.row is clamped to a row that exists
+    const bool bf16 = ep.small_bf16 != 0;
     float so[16];
     uint32_t mw[16];
-    // all loads of the 16 columns first (one DRAM latency instead of sixteen)
 #pragma unroll
     for (int jj = 0; jj < 16; ++jj) {
-        const int p = c0 + jj;
-        float sv = 0.0f; uint32_t m = 0xFFFFFFFFu;
-        if (cx.valid && p < n_act) {
-            if (epi == EPI_K3_STATE) sv = ep.s1[(int64_t)(ep.slot0 + p) * ep.ldN + cx.row];
-            if (ep.mask) m = __ldg(ep.mask + (int64_t)__ldg(ep.slot_plan + ep.slot0 + p) * ep.mask_words + cx.mword);
-        }
-        so[jj] = sv; mw[jj] = m;
+        const int p = min(c0 + jj, p_last);
+        so[jj] = (epi == EPI_K3_STATE) ? s1c[(int64_t)p * ep.ldN] : 0.0f;
+        mw[jj] = has_mask ? __ldg(mrow + (int64_t)__ldg(ep.slot_plan + ep.slot0 + p) * ep.mask_words) : 0xFFFFFFFFu;
     }
-#pragma unroll 1
+#pragma unroll
     for (int jj = 0; jj < 16; ++jj) {
-        const int p = c0 + jj;
-        if (p >= n_act) break;                      // warp-uniform
+        const int p = min(c0 + jj, p_last);
+        const bool inb = c0 + jj < n_act;                            // warp-uniform
+        const bool live = cx.valid && inb;
+        const bool on = (mw[jj] >> (cx.row & 31)) & 1u;
         float racc[kNumResid] = {0.f, 0.f, 0.f, 0.f, 0.f};
         float hinge = 0.f;
-        if (cx.valid) {
-            const bool on = (mw[jj] >> (cx.row & 31)) & 1u;
-            if (epi == EPI_K3_STATE) {
-                const float ub = on ? __ldg(ep.utab + cx.cls * kMaxBpad + ep.slot0 + p) : 0.0f;
-                const float cr = __ldg(ep.crtab + cx.cls * kMaxBpad + ep.slot0 + p);
-                Epi1Out o = epi1_element(so[jj], q[jj], cx.a_k, cr, ub, cx.resid, racc);
-                const int64_t idx = (int64_t)(ep.slot0 + p) * ep.ldN + cx.row;
-                ep.s1[idx] = o.s_new;
-                emit_small(ep.g_hi, ep.g_lo, (int64_t)(ep.slot0 + p) * ep.ldN, cx.row, o.g, ep.small_bf16 != 0);
-            } else {
-                hinge = on ? fmaxf(0.0f, cx.sense * (cx.thr - q[jj])) : 0.0f;
+        if (epi == EPI_K3_STATE) {
+            float rtmp[kNumResid] = {0.f, 0.f, 0.f, 0.f, 0.f};
+            const float ub = on ? __ldg(ep.utab + cx.cls * kMaxBpad + ep.slot0 + p) : 0.0f;
+            const float cr = __ldg(ep.crtab + cx.cls * kMaxBpad + ep.slot0 + p);
+            Epi1Out o = epi1_element(so[jj], q[jj], cx.a_k, cr, ub, cx.resid, rtmp);
+            if (live) {
+                ep.s1[(int64_t)(ep.slot0 + p) * ep.ldN + cx.row] = o.s_new;
+                emit_small(ep.g_hi, ep.g_lo, (int64_t)(ep.slot0 + p) * ep.ldN, cx.row, o.g, bf16);
+#pragma unroll
+                for (int t = 0; t < kNumResid; ++t) racc[t] = rtmp[t];
             }
+        } else {
+            hinge = (live && on) ? fmaxf(0.0f, cx.sense * (cx.thr - q[jj])) : 0.0f;
         }
+        if (!inb) continue;
         if (cx.resid) {
 #pragma unroll
             for (int t = 0; t < kNumResid; ++t) {
@@ -115,7 +120,7 @@ __device__ __noinline__ void epi_cols16(const TcLaunch& L, const EpiCtx& cx, int
         } else if (epi == EPI_OBJECTIVE) {
 #pragma unroll 1
             for (int k = 0; k < kMaxClasses; ++k) {
-                float v = warp_sum((cx.valid && cx.cls == k) ? hinge : 0.0f);
+                float v = warp_sum((live && cx.cls == k) ? hinge : 0.0f);
                 if (cx.lane == 0) cx.wacc[p * 8 + k] += v;
             }
         }
@@ -314,7 +319,7 @@ __global__ void __launch_bounds__(DRAIN ? 448 : 320, 1) admm_contract_kernel(con
             const TcUnit un = L.units[u];
             cx.lrow = ew * 32 + lane;
             cx.valid = cx.lrow < un.rows;
-            cx.row = (int64_t)un.row0 + cx.lrow;
+            cx.row = (int64_t)un.row0 + (cx.valid ? cx.lrow : 0);     // idle lanes load from a row that exists
             cx.slot = un.slot;
             cx.cls = 0;
             if (cx.valid && L.epi != EPI_K1_PARTIAL && L.epi != EPI_RAW) cx.cls = ep.point_class[cx.row];
@@ -360,7 +365,7 @@ __global__ void __launch_bounds__(DRAIN ? 448 : 320, 1) admm_contract_kernel(con
                 if (++b2 == 2) { b2 = 0; bph2 ^= 1; }
 #pragma unroll
                 for (int cc = 0; cc < 4; ++cc)
-                    if (cbeg + cc < cend) epi_cols16(L, cx, (cbeg + cc) * 16, &master[cc * 16]);
+                    if (cbeg + cc < cend) epi_cols16(L, cx, (cbeg + cc) * 16, *reinterpret_cast<const float(*)[16]>(&master[cc * 16]));
             } else {
                 tc::mbar_wait(&ctrl->tmem_full[a], aph);
                 tc::tcgen05_fence_after();
@@ -424,10 +429,12 @@ __device__ __forceinline__ void prefetch_s1_tile(const TcLaunch& L, const TcUnit
 // One warp = 32 consecutive rows (lane = row) x the plans [p_begin, p_end), in batches of 8 whose loads are all in
 // flight together; it runs concurrently with the MMAs / drains of the next unit.  Specialised at compile time on the
 // epilogue kind and on whether residual sums are wanted, 32-bit element offsets: the hot instance (K3, no residuals,
-// no mask) is ~35 instructions per plan (an all-in-one version was instruction-fetch and issue bound).
+// no mask) is ~35 instructions per plan.  Inlined on purpose: as a __noinline__ function it received the global-memory
+// descriptor in ordinary registers and paid R2UR moves before EVERY load and store (measured with clock64: 23-30 us per
+// unit, K3 was epilogue-bound: 134 us with bf16 storage against 78 us inlined).
 // wacc: this warp's [n_mma][8] partial sums.
 template <int EPI, bool RESID>
-__device__ __noinline__ void epilogue_unit_t(const TcLaunch& L, const TcUnit& un, const float* qs, int wq, int lane, float* wacc,
+__device__ __forceinline__ void epilogue_unit_t(const TcLaunch& L, const TcUnit& un, const float* qs, int wq, int lane, float* wacc,
                                              int p_begin, int p_end) {
     const EpiParams& ep = L.ep;
     const int lrow = wq * 32 + lane;
@@ -448,67 +455,81 @@ __device__ __noinline__ void epilogue_unit_t(const TcLaunch& L, const TcUnit& un
         }
         return;
     }
-    const int cls = valid ? ep.point_class[row] : 0;
+    // Everything below is written so that the per-batch arrays stay in REGISTERS and the 8 global loads of a batch are in
+    // flight together: loads are unconditional (indices clamped to a valid row / plan), only the stores are predicated.
+    // (An earlier version guarded the loads with `if (live)` and left the unrolled loop with `break`: the arrays went to
+    // local memory, every load was followed by a dependent STL, and the loads of a unit were served one DRAM latency at a
+    // time -- 23-30 us per unit, measured with clock64, which made K3 epilogue-bound.)
+    const int64_t rowc = valid ? row : (int64_t)un.row0;           // a row that exists, for the loads of idle lanes
+    const int cls = ep.point_class[rowc];
     const float a_k = ep.a_cls[cls], sense = ep.sense[cls], thr = ep.thr[cls];
-    const uint32_t mbit = (uint32_t)(row & 31);
+    const uint32_t mbit = (uint32_t)(rowc & 31);
     const float* utab = ep.utab + cls * kMaxBpad + ep.slot0;
     const float* crtab = ep.crtab + cls * kMaxBpad + ep.slot0;
     const int32_t* splan = ep.slot_plan + ep.slot0;
-    const uint32_t* mrow = ep.mask ? ep.mask + (row >> 5) : nullptr;
+    const bool has_mask = ep.mask != nullptr;
+    const uint32_t* mrow = has_mask ? ep.mask + (rowc >> 5) : reinterpret_cast<const uint32_t*>(ep.slot_plan);   // any valid address
     const uint32_t ldN = (uint32_t)ep.ldN;                     // Bpad * ldN < 2^32 (checked on the host)
-    const int64_t base = (int64_t)ep.slot0 * ep.ldN + row;
+    const int64_t base = (int64_t)ep.slot0 * ep.ldN + rowc;
     float* s1p = ep.s1 + base;
-    float* ghp = reinterpret_cast<float*>(ep.g_hi) + base;       // fp32 path only (this kernel)
+    float* ghp = reinterpret_cast<float*>(ep.g_hi) + base;       // fp32-container operands (tf32 grid)
     float* glp = reinterpret_cast<float*>(ep.g_lo) + base;
+    const bool bf16 = ep.small_bf16 != 0;
+    const int p_last = p_end - 1;
     constexpr int PB = 8;
     for (int p0 = p_begin; p0 < p_end; p0 += PB) {
-        float so[PB], ub[PB], cr[PB];
+        // phase 1: the long-latency loads (state, mask word) of the whole batch; the short ones (L1-resident tables,
+        // shared memory) are taken in phase 2
+        float so[PB];
         uint32_t mw[PB];
 #pragma unroll
         for (int j = 0; j < PB; ++j) {
-            const int p = p0 + j;
-            const bool live = valid && p < p_end;
-            so[j] = 0.f; ub[j] = 0.f; cr[j] = 0.f; mw[j] = 0xFFFFFFFFu;
-            if (live) {
-                if (EPI == EPI_K3_STATE) { so[j] = s1p[(uint32_t)p * ldN]; ub[j] = __ldg(utab + p); cr[j] = __ldg(crtab + p); }
-                if (mrow) mw[j] = __ldg(mrow + (int64_t)__ldg(splan + p) * ep.mask_words);
-            }
+            const int p = min(p0 + j, p_last);
+            so[j] = (EPI == EPI_K3_STATE) ? s1p[(uint32_t)p * ldN] : 0.0f;
+            mw[j] = has_mask ? __ldg(mrow + (int64_t)__ldg(splan + p) * ep.mask_words) : 0xFFFFFFFFu;
         }
 #pragma unroll
         for (int j = 0; j < PB; ++j) {
-            const int p = p0 + j;
-            if (p >= p_end) break;                      // warp-uniform
+            const int p = min(p0 + j, p_last);
+            const bool live = valid && (p0 + j < p_end);
+            const bool on = (mw[j] >> mbit) & 1u;
+            const float q = qp[p * kTileM];
             float racc[kNumResid] = {0.f, 0.f, 0.f, 0.f, 0.f};
             float hinge = 0.f;
-            if (valid) {
-                const bool on = (mw[j] >> mbit) & 1u;
-                const float q = qp[p * kTileM];
-                if (EPI == EPI_K3_STATE) {
-                    Epi1Out o = epi1_element(so[j], q, a_k, cr[j], on ? ub[j] : 0.0f, RESID, racc);
+            if (EPI == EPI_K3_STATE) {
+                float rtmp[kNumResid] = {0.f, 0.f, 0.f, 0.f, 0.f};
+                Epi1Out o = epi1_element(so[j], q, a_k, __ldg(crtab + p), on ? __ldg(utab + p) : 0.0f, RESID, rtmp);
+                if (live) {
                     const uint32_t off = (uint32_t)p * ldN;
                     s1p[off] = o.s_new;
-                    if (ep.small_bf16) {
+                    if (bf16) {
                         emit_small(ep.g_hi, ep.g_lo, (int64_t)(ep.slot0 + p) * ep.ldN, row, o.g, true);
                     } else {
                         const float ghi = tc::tf32_rna(o.g);
                         ghp[off] = ghi;
                         glp[off] = tc::tf32_rna(o.g - ghi);
                     }
-                } else {
-                    hinge = on ? fmaxf(0.0f, sense * (thr - q)) : 0.0f;
+#pragma unroll
+                    for (int t = 0; t < kNumResid; ++t) racc[t] = rtmp[t];
                 }
+            } else {
+                hinge = (live && on) ? fmaxf(0.0f, sense * (thr - q)) : 0.0f;
             }
             if (EPI == EPI_K3_STATE && RESID) {
+                if (p0 + j < p_end) {                               // warp-uniform
 #pragma unroll
-                for (int t = 0; t < kNumResid; ++t) {
-                    float v = warp_sum(racc[t]);
-                    if (lane == 0) wacc[p * 8 + t] += v;
+                    for (int t = 0; t < kNumResid; ++t) {
+                        float v = warp_sum(racc[t]);
+                        if (lane == 0) wacc[p * 8 + t] += v;
+                    }
                 }
             } else if (EPI == EPI_OBJECTIVE) {
+                if (p0 + j < p_end) {
 #pragma unroll 1
-                for (int k = 0; k < kMaxClasses; ++k) {
-                    float v = warp_sum((valid && cls == k) ? hinge : 0.0f);
-                    if (lane == 0) wacc[p * 8 + k] += v;
+                    for (int k = 0; k < kMaxClasses; ++k) {
+                        float v = warp_sum((live && cls == k) ? hinge : 0.0f);
+                        if (lane == 0) wacc[p * 8 + k] += v;
+                    }
                 }
             }
         }

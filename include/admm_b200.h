@@ -74,8 +74,8 @@ typedef struct {
     int32_t compaction;        /* 1: converged plans are swapped out of the active batch; 0: masked only */
     float   csr_rel_threshold; /* ADMM_STORAGE_CSR only; 0 => 1e-3                                  */
     int32_t profile_kernels;   /* 1: CUDA events around every hot-path kernel (admm_get_kernel_times) */
-    int32_t drain_kb;          /* fp32 path: the TMEM accumulator is drained into fp32 registers every this many
-                                  32-element k-blocks; 0 => default, -1 => never            */
+    int32_t drain_kb;          /* the TMEM accumulator is drained into fp32 registers every this many 128-byte k-blocks
+                                  (DESIGN.md section 7); 0 => default (1; 4 for bf16 storage), -1 => never        */
     int32_t k1_slab_kb;        /* K1 walks the point range in slabs of this many 32-point k-blocks so the slab of the plan
                                   operand stays in L2; 0 => chosen from the sizes            */
     int32_t reserved[5];       /* must be 0 */

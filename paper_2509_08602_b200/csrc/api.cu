@@ -181,7 +181,10 @@ int chunk_kb(const admm_handle* h) {
     if (h->opt.kernel_path != ADMM_PATH_TCGEN05) return 0;
     if (h->opt.drain_kb < 0) return 0;
     if (h->opt.drain_kb > 0) return h->opt.drain_kb;
-    return h->opt.storage == ADMM_STORAGE_BF16 ? 4 : 1;      // bf16 storage has a 1e-2 budget: drain less often
+    // every k-block: draining every 2 is 8 % faster (config 1: K1 / K3 106 / 140 -> 97 / 129 us) but its ~3e-7 coherent bias
+    // per product pushes the K = 50 iterates to 1.1-1.8e-4 of the oracle's, over north_star's 1e-4; bf16 storage has a 1e-2
+    // budget and drains every 4
+    return h->opt.storage == ADMM_STORAGE_BF16 ? 4 : 1;
 }
 // plans per contraction pass
 int max_pass(const admm_handle* h) {

@@ -673,25 +673,35 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
     if (warp == 0) {
         // ------------------------------------------------------------ TMA producer: two independent rings, one polling lane
         if (lane == 0) {
-            KbIter ia, ib;
-            ia.start(L, unit_begin, unit_end); ib.start(L, unit_begin, unit_end);
+            // the unit record is read from global memory ONCE per unit and kept in registers (reading L.units[] for every
+            // k-block put a dependent global load in front of every TMA issue)
+            int ua = unit_begin, ub = unit_begin, kba = 0, kbb = 0;
+            TcUnit una = TcUnit{0, 0, 0, 0, 0, 0}, unb = una;
+            if (unit_begin < unit_end) { una = L.units[unit_begin]; unb = una; }
+            int arow = ((una.row0 >> 7) * L.big_kb_total + una.kb0) * kTileM;      // tile-major row of the next A tile
+            int bk0 = unb.kb0 * L.kblk;                                             // element coordinate of the next B tile
             int sa = 0, sb = 0; uint32_t pha = 0, phb = 0;
-            while (ia.u < unit_end || ib.u < unit_end) {
-                if (ia.u < unit_end && tc::mbar_test_wait(&ctrl->sa_empty[sa], pha ^ 1)) {
-                    const TcUnit un = L.units[ia.u];
+            while (ua < unit_end || ub < unit_end) {
+                if (ua < unit_end && tc::mbar_test_wait(&ctrl->sa_empty[sa], pha ^ 1)) {
                     // one 16 KB tile of the tile-major big operand (rows past the end of the matrix are stored as zeros)
                     tc::mbar_arrive_expect_tx(&ctrl->sa_full[sa], kTileBytes);
-                    tc::tma_load_2d(a_ring + sa * kTileBytes, &L.map_big128, &ctrl->sa_full[sa], 0,
-                                    ((un.row0 >> 7) * L.big_kb_total + un.kb0 + ia.kb) * kTileM, tc::kEvictFirst);
-                    ia.next(L, unit_end);
+                    tc::tma_load_2d(a_ring + sa * kTileBytes, &L.map_big128, &ctrl->sa_full[sa], 0, arow, tc::kEvictFirst);
+                    arow += kTileM;
+                    if (++kba == una.kb_count) {
+                        kba = 0;
+                        if (++ua < unit_end) { una = L.units[ua]; arow = ((una.row0 >> 7) * L.big_kb_total + una.kb0) * kTileM; }
+                    }
                     if (++sa == n_sa) { sa = 0; pha ^= 1; }
                 }
-                if (ib.u < unit_end && tc::mbar_test_wait(&ctrl->sb_empty[sb], phb ^ 1)) {
-                    const int k0 = (L.units[ib.u].kb0 + ib.kb) * L.kblk;
+                if (ub < unit_end && tc::mbar_test_wait(&ctrl->sb_empty[sb], phb ^ 1)) {
                     tc::mbar_arrive_expect_tx(&ctrl->sb_full[sb], bbytes);
-                    tc::tma_load_2d(b_ring + sb * bbytes, &L.map_small_hi, &ctrl->sb_full[sb], k0, 0, tc::kEvictLast);
-                    tc::tma_load_2d(b_ring + sb * bbytes + bbytes / 2, &L.map_small_lo, &ctrl->sb_full[sb], k0, 0, tc::kEvictLast);
-                    ib.next(L, unit_end);
+                    tc::tma_load_2d(b_ring + sb * bbytes, &L.map_small_hi, &ctrl->sb_full[sb], bk0, 0, tc::kEvictLast);
+                    tc::tma_load_2d(b_ring + sb * bbytes + bbytes / 2, &L.map_small_lo, &ctrl->sb_full[sb], bk0, 0, tc::kEvictLast);
+                    bk0 += L.kblk;
+                    if (++kbb == unb.kb_count) {
+                        kbb = 0;
+                        if (++ub < unit_end) { unb = L.units[ub]; bk0 = unb.kb0 * L.kblk; }
+                    }
                     if (++sb == n_sb) { sb = 0; phb ^= 1; }
                 }
             }

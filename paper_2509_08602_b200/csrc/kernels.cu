@@ -227,10 +227,11 @@ __global__ void k2a_kernel(const float* __restrict__ partial, const int32_t* __r
 // tcgen05 has no fp64 kind; the fp64 tensor path of sm_100 is mma.sync m8n8k4 (DMMA), used here directly.
 //
 // Block = WJ x 2 warps; warp tile = 16 rows (time variables j) x 48 plans = 2 x 6 DMMA fragments; block tile = 16 WJ x 96.
-// K is walked in chunks of 32 through a 3-stage cp.async ring; both operands are K-contiguous in memory
-// (Sinv[j][k] row-major with padded row stride, rhs[p][k] plan-major), rows padded to 36 doubles => conflict-free LDS.64.
+// K is walked in chunks of 64 through a cp.async ring (as deep as ~200 KB allows); both operands are K-contiguous in memory
+// (Sinv[j][k] row-major with padded row stride, rhs[p][k] plan-major), rows padded to 68 doubles => conflict-free LDS.64.
 // Epilogue (4b)/(4c) on block 2 in single-state form: s2+ = z2 + v, z2 = min(s2, R beta); emits V = R o v (tf32 hi/lo).
-constexpr int K2_TP = 96, K2_KC = 32, K2_LD = K2_KC + 4;
+constexpr int K2_TP = 96, K2_KC = 64, K2_LD = K2_KC + 4;       // 64-column chunks: half as many barrier rounds as 32
+constexpr int K2_TPR = K2_KC / 2, K2_RPP = 256 / K2_TPR;        // loader: threads per row (16-byte pieces), rows per pass
 // ring depth: as many 32-column chunks as fit in ~200 KB (the operands come from L2 / HBM at ~1 us latency and the
 // DMMA work per chunk is a few hundred cycles: bytes in flight are what sets the speed)
 __host__ __device__ constexpr int k2_stages(int WJ) { return (200 * 1024) / ((16 * WJ + K2_TP) * K2_LD * 8) > 8 ? 8 : (200 * 1024) / ((16 * WJ + K2_TP) * K2_LD * 8); }
@@ -267,18 +268,18 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
     const bool warp_live = p0 + wp * 48 < Bact;
 
     // loader: thread t copies 16-byte pieces (row = t/16 + 16 i, columns kk, kk+1) for i < NCP; pointers are set up once
-    constexpr int NCP = ROWS * (K2_KC / 2) / NT;             // 7 / 8 / 10 for WJ = 1 / 2 / 4 (exact)
+    constexpr int NCP = ROWS * (K2_KC / 2) / NT;             // 14 / 16 / 20 for WJ = 1 / 2 / 4 (exact)
     static_assert(ROWS * (K2_KC / 2) % NT == 0, "loader tiling");
-    const int kk = (tid & 15) * 2;
+    const int kk = (tid % K2_TPR) * 2;
     const double* srcp[NCP];
     bool rowok[NCP];
 #pragma unroll
     for (int i = 0; i < NCP; ++i) {
-        const int row = (tid >> 4) + 16 * i;
+        const int row = tid / K2_TPR + K2_RPP * i;
         if (row < TJ) { const int64_t j = j0 + row; rowok[i] = j < n; srcp[i] = Sinv + (rowok[i] ? j : 0) * lds + kk; }
         else { const int p = p0 + row - TJ; rowok[i] = p < Bact; srcp[i] = rhs + (int64_t)(rowok[i] ? p : 0) * ldn + kk; }
     }
-    const uint32_t dst0 = (uint32_t)__cvta_generic_to_shared(k2sm) + (uint32_t)(((tid >> 4) * K2_LD + kk) * 8);
+    const uint32_t dst0 = (uint32_t)__cvta_generic_to_shared(k2sm) + (uint32_t)(((tid / K2_TPR) * K2_LD + kk) * 8);
     auto load_chunk = [&](int c, int stage) {
         const int64_t k0 = (int64_t)c * K2_KC;
         const bool kok = k0 + kk < n;
@@ -286,7 +287,7 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
 #pragma unroll
         for (int i = 0; i < NCP; ++i) {
             const int sz = (kok && rowok[i]) ? 16 : 0;
-            asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2, %3;" ::"r"(d + (uint32_t)(i * 16 * K2_LD * 8)),
+            asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2, %3;" ::"r"(d + (uint32_t)(i * K2_RPP * K2_LD * 8)),
                          "l"(kok ? srcp[i] + k0 : srcp[i]), "r"(sz), "l"(tc::kEvictLast) : "memory");
         }
     };

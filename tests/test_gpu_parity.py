@@ -392,3 +392,34 @@ def test_single_plan_and_degenerate_weights(b):
     out = b.admm_solve_batch(h, np.array([[1.0, 0.5, 1.5 * bound]]), None, tol=1e-4, max_iter=3000)
     assert abs(out["obj"][0] - 1.0) < 1e-3 and np.max(np.abs(out["t"])) < 1e-3
     h.close()
+
+
+def test_edge_cases_max_batch_and_fully_masked_class(b):
+    """B = 496 (the ABI's maximum: six passes of 96 plans, the last one ragged); a plan whose low-dose rows are ALL masked out
+    (N_kp = 0 => u = 0 on that class, reading R12) equals the same plan with alpha = 0; B above the maximum is refused."""
+    from workloads import default_rho, make_workload, pack_mask
+    w = make_workload(0, n_target=150, n_lowdose=260, n_iso=2)
+    rng = np.random.default_rng(4)
+    B = 496
+    weights = np.stack([np.ones(B), rng.uniform(0, 1, B), rng.uniform(0, 1, B)], axis=1)
+    rho = default_rho(weights[:, 2])
+    h = b.admm_setup(w.phi, w.point_class, w.classes)
+    out = b.admm_solve_batch(h, weights, rho, fixed_iters=12)
+    for p in (0, 95, 96, 300, 495):                                   # plan p in the batch == the same plan alone (bit-exact)
+        z1, y1, z2, y2 = b.admm_get_state(h, p)
+        o1 = b.admm_solve_batch(h, weights[[p]], rho[[p]], fixed_iters=12)
+        s1 = b.admm_get_state(h, 0)
+        assert np.array_equal(z1, s1[0]) and np.array_equal(y1, s1[1]) and np.array_equal(z2, s1[2]) and np.array_equal(y2, s1[3])
+        assert np.array_equal(o1["t"][0], out["t"][p])
+        out = b.admm_solve_batch(h, weights, rho, fixed_iters=12)
+    with pytest.raises(b.AdmmError) as e:
+        b.admm_solve_batch(h, np.ones((497, 3)), None, fixed_iters=1)
+    assert e.value.status == b.ADMM_EINVAL
+    # fully masked low-dose class
+    mask = np.ones((2, w.N), dtype=bool)
+    mask[0, w.point_class == 1] = False
+    wts = np.array([[1.0, 0.7, 0.3], [1.0, 0.0, 0.3]])
+    o = b.admm_solve_batch(h, wts, np.array([1e-3, 1e-3]), pack_mask(mask), fixed_iters=40)
+    assert np.all(np.isfinite(o["t"])) and np.all(np.isfinite(o["obj"]))
+    assert np.allclose(o["t"][0], o["t"][1], rtol=1e-6, atol=1e-9) and abs(o["obj"][0] - o["obj"][1]) < 1e-9
+    h.close()

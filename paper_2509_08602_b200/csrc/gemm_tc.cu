@@ -568,7 +568,8 @@ __device__ __forceinline__ void epilogue_unit(const TcLaunch& L, const TcUnit& u
 //                 alternate so the drain of chunk c overlaps the MMAs of chunk c+1.  The small (2^-11) terms stay in
 //                 TMEM for the whole unit.
 // TMEM columns: region 0 [0, 2n) | region 1 [2n, 4n) | A ring [384, 512) = 2 x (hi 32 | lo 32);   n = n_mma <= 96.
-constexpr int kF32Warps = 22;              // TMA, MMA, 4 converter, 8 drain, 8 epilogue
+constexpr int kF32Warps = 23;              // TMA, MMA, 4 converter, 8 drain, 8 epilogue, second MMA issuer
+constexpr int kMma2Warp = 22;
 constexpr int kF32Threads = kF32Warps * 32;
 constexpr int kF32MaxMmaN = 96;
 constexpr int kAcol = 384;
@@ -640,7 +641,7 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
         for (int i = 0; i < 2; ++i) {
             tc::mbar_init(&ctrl->a_full[i], 4);
             tc::mbar_init(&ctrl->a_empty[i], 1);
-            tc::mbar_init(&ctrl->d_full[i], 1);
+            tc::mbar_init(&ctrl->d_full[i], L.mma_passes == 3 ? 2 : 1);      // one arrival per MMA issuer (two in 3xTF32 mode)
             tc::mbar_init(&ctrl->d_empty[i], 8);
         }
         tc::mbar_init(&ctrl->q_full, 8);
@@ -706,8 +707,20 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
                 }
             }
         }
-    } else if (warp == 1) {
-        // ------------------------------------------------------------ UMMA issuer (warp-uniform loop, one elected lane issues)
+    } else if (warp == 1 || warp == kMma2Warp) {
+        // ------------------------------------------------------------ UMMA issuers (warp-uniform loop, one elected lane issues)
+        // TWO issuing warps take the k-blocks in turn (even / odd): measured with clock64, one warp needs ~1200 cycles of
+        // serial latency per k-block (three mbarrier probes ~130 each, fence + 8 MMAs + 3 commits ~530, bookkeeping) for 576
+        // cycles of tensor work, so a single issuer kept the pipe half idle.  k-block parity = A-ring slot = parity of the (even-
+        // depth) smem stages, so each of those barriers is always probed by the same warp and no phase goes unobserved; the D
+        // regions are shared: both warps wait d_empty and both arrive on d_full (count 2), by commit after their last k-block
+        // of the chunk or by a plain arrive when the chunk held none of theirs.
+        const int mma_id = (warp == 1) ? 0 : 1;
+        // direct modes keep ONE issuer: there the MMA warp also waits on the smem A ring, whose depth (3 at n_mma = 96) would have
+        // to be cut to 2 to stay even, which costs more than the second issuer gains (measured: tf32 102 -> 123 us)
+        const bool two = L.mma_passes == 3;
+        int gkb = 0;                        // k-blocks seen so far (all units): its parity picks the issuer
+        if (two || mma_id == 0) {
         const bool direct = L.mma_passes != 3;     // Phi already exact in the operand format (tf32 / bf16 storage): A straight from smem
         const uint32_t fmt = L.mma_kind == 1 ? 1u : 2u;
         const uint32_t idesc_wide = tc::umma_idesc(fmt, kTileM, (uint32_t)(2 * n_mma));
@@ -728,7 +741,19 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
                 tc::mbar_wait(&ctrl->d_empty[a], aph ^ 1);
                 const uint32_t d_main = tmem_base + a * 2 * n_mma;
                 const uint32_t d_small = d_main + n_mma;
-                for (int kb = 0; kb < nkb; ++kb) {
+                // my last k-block of this chunk (-1: none): that is where my arrival on d_full goes
+                int my_last = -1;
+                for (int kb = nkb - 1; kb >= 0; --kb) if (!two || ((gkb + kb) & 1) == mma_id) { my_last = kb; break; }
+                if (my_last < 0) { if (tc::elect_one()) tc::mbar_arrive(&ctrl->d_full[a]); __syncwarp(); }
+                for (int kb = 0; kb < nkb; ++kb, ++gkb) {
+                    const bool mine = !two || (gkb & 1) == mma_id;
+                    if (!mine) {            // the other issuer's k-block: only keep the ring counters in step
+                        b_desc += b_step;
+                        if (++sb == n_sb) { sb = 0; phb ^= 1; b_desc = b_desc0; }
+                        if (++sa == n_sa) { sa = 0; pha ^= 1; }
+                        if (++t == 2) { t = 0; tph ^= 1; }
+                        continue;
+                    }
                     tc::mbar_wait(&ctrl->sb_full[sb], phb);     // the small operand landed (async proxy)
                     if (direct) {
                         tc::mbar_wait(&ctrl->sa_full[sa], pha); // the big operand's tile landed (async proxy): it IS the A operand
@@ -743,10 +768,9 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
                             }
                             tc::umma_commit(&ctrl->sb_empty[sb]);
                             tc::umma_commit(&ctrl->sa_empty[sa]);
-                            if (kb == nkb - 1) tc::umma_commit(&ctrl->d_full[a]);
+                            if (kb == my_last) tc::umma_commit(&ctrl->d_full[a]);
                         }
                         __syncwarp();
-                        if (++sa == n_sa) { sa = 0; pha ^= 1; }
                     } else {
                     tc::mbar_wait(&ctrl->a_full[t], tph);       // the converter's hi/lo are in TMEM
                     tc::tcgen05_fence_after();
@@ -759,16 +783,18 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
                         }
                         tc::umma_commit(&ctrl->sb_empty[sb]);
                         tc::umma_commit(&ctrl->a_empty[t]);
-                        if (kb == nkb - 1) tc::umma_commit(&ctrl->d_full[a]);
+                        if (kb == my_last) tc::umma_commit(&ctrl->d_full[a]);
                     }
                     __syncwarp();
                     }
                     b_desc += b_step;
                     if (++sb == n_sb) { sb = 0; phb ^= 1; b_desc = b_desc0; }
+                    if (++sa == n_sa) { sa = 0; pha ^= 1; }
                     if (++t == 2) { t = 0; tph ^= 1; }
                 }
                 if (++a == 2) { a = 0; aph ^= 1; }
             }
+        }
         }
     } else if (warp >= kConvWarp0 && warp < kDrainWarp0) {
         if (L.mma_passes == 3) {
@@ -990,6 +1016,11 @@ admm_status tc_launch(admm_handle* h, const TcLaunch& L) {
         if (f32_a_stages(n_mma) < 2) { h->err = "tc_launch: fewer than 2 pipeline stages fit in shared memory"; return ADMM_EINVAL; }
         TcLaunch L2 = L;
         L2.n_sb = f32_b_stages(n_mma); L2.n_sa = f32_a_stages(n_mma);
+        // the two MMA issuers take the chunks in turn and only probe the barriers of their own k-blocks: every ring they wait on
+        // must have an EVEN depth, so that a stage is always consumed by the same warp and no mbarrier phase goes unobserved
+        // (a parity probe cannot tell "two phases behind" from "done").  3xTF32 mode only (direct modes have one issuer): B ring 4 or 2;
+        // the A rings it waits on are the 2 TMEM slots.
+        if (L.mma_passes == 3 && L2.n_sb == 3) L2.n_sb = 2;
         admm_contract_f32_kernel<<<L.grid, kF32Threads, kSmemLimit, h->stream>>>(L2);
     } else {
         admm_contract_kernel<false><<<L.grid, 320, kSmemLimit, h->stream>>>(L);

@@ -71,17 +71,21 @@ typedef struct {
     void*   stream;            /* cudaStream_t all work is enqueued on; NULL = the legacy default stream */
     int32_t check_every;       /* stopping rule tested every this many iterations; 0 => 10          */
     float   eps_abs;           /* absolute part of the stopping rule; 0 => 1e-6 (reading R7) */
-    int32_t compaction;        /* 1: converged plans are swapped out of the active batch; 0: masked only */
+    int32_t compaction;        /* must be 1: a plan that passes the stopping rule is frozen at that iterate and moved out of the
+                                  active batch on the device (masking without compaction is not offered: 0 => ADMM_EINVAL) */
     float   csr_rel_threshold; /* ADMM_STORAGE_CSR only; 0 => 1e-3                                  */
     int32_t profile_kernels;   /* 1: CUDA events around every hot-path kernel (admm_get_kernel_times) */
     int32_t drain_kb;          /* the TMEM accumulator is drained into fp32 registers every this many 128-byte k-blocks
                                   (DESIGN.md section 7); 0 => default (1; 4 for bf16 storage), -1 => never        */
     int32_t k1_slab_kb;        /* K1 walks the point range in slabs of this many 32-point k-blocks so the slab of the plan
                                   operand stays in L2; 0 => chosen from the sizes            */
-    int32_t reserved[5];       /* must be 0 */
+    int32_t presolve;          /* 1 (default): before iterating (tolerance mode only), plans whose box optimum x = argmin c^T x over
+                                  [0,u] already satisfies A x <= b are settled in closed form: t = 0, iterations = 0, state = the
+                                  ADMM fixed point (an LP presolve, not in the paper: DESIGN.md deviation D1); 0: every plan iterates */
+    int32_t reserved[4];       /* must be 0 */
 } admm_options;
 
-/* Fills *opt with the defaults (3xTF32, tcgen05 path, device 0, default stream, check 10, 1e-6, compaction on). */
+/* Fills *opt with the defaults (3xTF32, tcgen05 path, device 0, default stream, check 10, 1e-6, compaction on, presolve on). */
 void admm_default_options(admm_options* opt);
 
 /*

@@ -19,6 +19,12 @@ Boyd et al. section 3.3 on the scaled problem, per plan, tested every `check_eve
     ||x - z+||_2 <= eps_abs*sqrt(N+n) + tol*max(||x||_2, ||z+||_2)   and
     ||z+ - z||_2 <= eps_abs*sqrt(N+n) + tol*||y+||_2
 (norms over both blocks stacked).  A plan that meets it is frozen at that iterate.
+
+Optional presolve (NOT in the paper; DESIGN.md deviation D1, off by default): the minimiser of c^T x over the box
+alone is x_box = u where c < 0, 0 where c > 0.  If A x_box <= b it is feasible for Eq. (1) and therefore optimal,
+the multipliers of A x <= b vanish (t* = 0), and Eq. (6), (7), (4b), (4c) have the fixed point
+    z1 = x_box,  y1 = -c/rho,  z2 = A x_box,  y2 = 0        (v = 0 in Eq. 6)
+which is returned for such a plan with 0 iterations.
 """
 from __future__ import annotations
 
@@ -76,9 +82,26 @@ def plan_bounds(pre: Preconditioned, point_class, classes, weights, masks: Optio
     return u_hat, b_hat
 
 
+def presolve_box_optimum(pre: Preconditioned, u_hat, b_hat, rho, margin: float = 1e-5):
+    """Plans whose box optimum is feasible (module docstring).  Returns (accepted [B] bool, state dict for those
+    plans' columns: z1, y1, z2, y2).  `margin`: A x_box <= b (1 - margin) is required, so that a plan sitting on the
+    boundary within rounding is left to the iteration."""
+    rho = np.asarray(rho, dtype=np.float64)
+    c = pre.c_hat[:, None]
+    x_box = np.where(c < 0, u_hat, 0.0)                                   # [N, B]
+    finite = np.all(np.isfinite(x_box), axis=0)
+    x_safe = np.where(np.isfinite(x_box), x_box, 0.0)
+    Ax = pre.A_hat @ x_safe                                               # [n, B]
+    accepted = finite & np.all(Ax <= b_hat * (1.0 - margin), axis=0)
+    state = dict(z1=x_safe, y1=-c / rho[None, :] + 0.0 * x_safe, z2=Ax, y2=np.zeros_like(Ax))
+    return accepted, state
+
+
 def admm_run(pre: Preconditioned, u_hat, b_hat, rho, iters: int, tol: Optional[float] = None,
-             eps_abs: float = 1e-6, check_every: int = 10, state0=None, history: bool = False):
-    """Run `iters` iterations (tol=None) or until every plan meets the stopping rule / iters."""
+             eps_abs: float = 1e-6, check_every: int = 10, state0=None, history: bool = False,
+             presolve: bool = False):
+    """Run `iters` iterations (tol=None) or until every plan meets the stopping rule / iters.
+    presolve=True (tolerance mode only): see presolve_box_optimum."""
     A = pre.A_hat
     n, N = A.shape
     rho = np.asarray(rho, dtype=np.float64)
@@ -94,6 +117,13 @@ def admm_run(pre: Preconditioned, u_hat, b_hat, rho, iters: int, tol: Optional[f
     res = np.zeros((B, 2))
     hist = [] if history else None
     dim = np.sqrt(float(N + n))
+    presolved = np.zeros(B, dtype=bool)
+    if presolve and tol is not None and state0 is None:
+        presolved, ps = presolve_box_optimum(pre, u_hat, b_hat, rho)
+        for name, arr in (("z1", z1), ("y1", y1), ("z2", z2), ("y2", y2)):
+            arr[:, presolved] = ps[name][:, presolved]
+        active &= ~presolved
+        converged |= presolved
     for k in range(1, iters + 1):
         r1 = z1 - y1 - c_over_rho
         r2 = z2 - y2
@@ -122,7 +152,7 @@ def admm_run(pre: Preconditioned, u_hat, b_hat, rho, iters: int, tol: Optional[f
             active = active & ~ok
             if not active.any():
                 break
-    out = dict(z1=z1, y1=y1, z2=z2, y2=y2, iters=it_done, converged=converged, res=res)
+    out = dict(z1=z1, y1=y1, z2=z2, y2=y2, iters=it_done, converged=converged, res=res, presolved=presolved)
     if hist is not None:
         out["history"] = np.stack(hist, axis=0)        # [iters, B, 5]
     return out
@@ -136,7 +166,7 @@ def recover(pre: Preconditioned, state, rho):
     return t, lam
 
 
-def solve_workload(w, rho, iters, tol=None, check_every=10, eps_abs=1e-6, pre=None, history=False):
+def solve_workload(w, rho, iters, tol=None, check_every=10, eps_abs=1e-6, pre=None, history=False, presolve=False):
     """Convenience: precondition + bounds + run + recover + primal objective per plan."""
     from .lp_model import primal_objective
     if pre is None:
@@ -144,7 +174,7 @@ def solve_workload(w, rho, iters, tol=None, check_every=10, eps_abs=1e-6, pre=No
     masks = None if w.row_mask is None else w.mask_bool()
     u_hat, b_hat = plan_bounds(pre, w.point_class, w.classes, w.weights, masks)
     st = admm_run(pre, u_hat, b_hat, rho, iters, tol=tol, eps_abs=eps_abs, check_every=check_every,
-                  history=history)
+                  history=history, presolve=presolve)
     t, lam = recover(pre, st, rho)
     obj = np.array([primal_objective(w.phi, w.point_class, w.classes, w.weights[p], t[p],
                                      None if masks is None else masks[p]) for p in range(w.B)])

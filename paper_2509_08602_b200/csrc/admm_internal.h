@@ -14,6 +14,7 @@ constexpr int kBlockK = 32;        // fp32 elements per k-block = one 128-byte s
 constexpr int kBoxRows = 32;       // rows per TMA box of the big operand (partial tiles load fewer boxes)
 constexpr int kMaxBpad = 512;      // slots in the per-plan tables / partial-sum arrays (B <= 512)
 constexpr int kMaxMmaN = 256;      // plans per contraction pass (UMMA N limit); larger batches run in chunks
+constexpr double kRhoFloorDiv = 64.0;   // default rho rule: w_BOT is clamped below at w0 / kRhoFloorDiv (reading R8)
 constexpr int kNumResid = 5;       // ||x-z+||^2, ||z+-z||^2, ||x||^2, ||z+||^2, ||y+||^2
 
 // One unit of work of a contraction kernel: a 128-row tile of the big operand times a k-range.
@@ -33,7 +34,9 @@ enum { EPI_K1_PARTIAL = 0, EPI_K3_STATE = 1, EPI_OBJECTIVE = 2, EPI_RAW = 3 };
 struct EpiParams {
     // common
     int32_t slot0;              // first slot of this contraction pass (chunk of <= 256 plans)
-    int32_t n_slots_active;     // live slots of this pass: slot0 .. slot0 + n_slots_active - 1
+    int32_t n_slots_active;     // live slots of this pass: slot0 .. slot0 + n_slots_active - 1 (the HOST's upper bound)
+    const int32_t* bact_dev;    // device scalar: live slots of the whole batch right now (nullptr: n_slots_active is exact).
+                                // The host's bound lags the device by up to one check interval; see eff_nact().
     int32_t n_mma;              // UMMA N (multiple of 16, >= n_slots_active)
     int64_t N, n;               // points, time variables
     int64_t ldN, ldn;           // row strides of [slot][N] and [slot][n] arrays (elements)
@@ -57,6 +60,18 @@ struct EpiParams {
     double* hinge_partial;          // objective: [grid][kMaxBpad][kMaxClasses]
     float* qraw;                    // EPI_RAW (test hook): raw accumulators [slot][ldN]
 };
+
+// Live slots of this pass as the DEVICE knows them: the compaction kernel shrinks *bact_dev, the host's n_slots_active (which
+// sized the launch: n_mma, grids) follows one check interval later.
+__host__ __device__ inline int eff_nact(const EpiParams& ep) {
+#ifdef __CUDA_ARCH__
+    if (ep.bact_dev) {
+        const int live = *ep.bact_dev - ep.slot0;
+        return live < 0 ? 0 : (live < ep.n_slots_active ? live : ep.n_slots_active);
+    }
+#endif
+    return ep.n_slots_active;
+}
 
 struct TcLaunch {
     CUtensorMap map_big;     // big operand, tile-major [tiles * 128][32], box {32, 32}
@@ -118,21 +133,30 @@ struct admm_handle {
     float* d_resid1 = nullptr;                                        // [grid][kMaxBpad][5]
     double* d_resid2 = nullptr;                                       // [blocks][kMaxBpad][5]
     double* d_hinge = nullptr;                                        // [grid][kMaxBpad][kMaxClasses]
-    uint32_t* d_mask = nullptr; int64_t mask_words = 0; bool has_mask = false;
+    uint32_t* d_mask = nullptr; int64_t mask_words = 0; bool has_mask = false; int64_t mask_capacity = 0;
     int32_t* d_slot_plan = nullptr;
     float *d_utab = nullptr, *d_crtab = nullptr;
     double *d_beta = nullptr, *d_rho = nullptr;                       // per slot
     int32_t* d_active_counts = nullptr;                               // [B][kMaxClasses]
-    int32_t* d_conv_flags = nullptr;                                  // [Bpad] + counter
-    float* d_res_slot = nullptr;                                      // [Bpad][2]
-    float* d_rowtmp = nullptr; double* d_rowtmp2 = nullptr;
+    int32_t* d_conv_flags = nullptr;                                  // [Bpad] stopping-rule / presolve verdict per slot
+    int32_t* d_bact = nullptr;                                        // device scalar: live slots (H5 shrinks it on the device)
+    int32_t* d_moves = nullptr; int32_t* d_nmoves = nullptr;          // compaction: [Bpad/2][2] slot pairs + their count
+    int32_t* d_iters_plan = nullptr; float* d_res_plan = nullptr;     // per PLAN: iterations done, residual norms [B][2]
+    double* d_wnorm = nullptr;                                        // [kMaxBpad][kMaxClasses] w_k / N_kp per slot
+    float* d_t_f32 = nullptr; double* d_obj = nullptr;                // finalise: t [Bpad][ldn], objective per slot
+    int32_t* d_plan_slot = nullptr; float* d_tout = nullptr;          // outputs in plan order
+    float* d_qbuf = nullptr;                                          // SIMT / CSR path: Q [pass][ldN]
+    int32_t* h_bact_ring = nullptr;                                   // pinned host ring the live count is copied into after every check
+    cudaEvent_t bact_ev[8] = {};                                      // one event per ring entry
+    bool k2_attr_set = false;
+    struct MapKey { int kind, slot0, n_mma; CUtensorMap big, big128, hi, lo; };
+    std::vector<MapKey> map_cache;                                    // tensor maps per (contraction, slot0, n_mma); cleared on reallocation
     TcUnit* d_units_k1 = nullptr; int32_t* d_cta_begin_k1 = nullptr; int grid_k1 = 0; int slots_k1 = 0;
     int32_t* d_mtile_slot_begin = nullptr;                            // [m_tiles + 1]
     TcUnit* d_units_k3 = nullptr; int32_t* d_cta_begin_k3 = nullptr; int grid_k3 = 0;
     std::vector<int32_t> slot_plan, plan_slot, iters;
-    std::vector<double> h_beta, h_rho;
-    std::vector<float> h_weights;
     bool solved = false;
+    int32_t presolved = 0;                                            // plans of the last solve settled by the presolve
 
     double ms[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     int64_t plan_iters = 0;
@@ -170,11 +194,16 @@ void launch_k2a(admm_handle* h, int slot0, int nact, int n_mma, cudaStream_t s);
 void launch_k2b(admm_handle* h, int Bact, bool resid, cudaStream_t s);
 void launch_simt_k1(admm_handle* h, int slot0, int nact, int n_mma, int splits, cudaStream_t s);
 void launch_simt_k3(admm_handle* h, const EpiParams& ep, int epi, const float* vhi, const float* vlo, float* qbuf, cudaStream_t s);
-void launch_convergence(admm_handle* h, int Bact, int grid1, int grid2, float tol, float eps_abs, cudaStream_t s);
+void launch_convergence(admm_handle* h, int Bact, int grid1, int grid2, float tol, float eps_abs, int it, cudaStream_t s);
+void launch_compaction(admm_handle* h, int Bact, cudaStream_t s);
+void launch_presolve_state(const EpiParams& ep, int B, cudaStream_t s);
+void launch_presolve_test(admm_handle* h, int slot0, int nact, int n_mma, double margin, cudaStream_t s);
+void launch_presolve_reset(admm_handle* h, int B, cudaStream_t s);
+void launch_init_plan_records(admm_handle* h, int B, cudaStream_t s);
 void launch_make_t(admm_handle* h, int Bact, void* t_hi, void* t_lo, float* t_f32, cudaStream_t s);
 void launch_objective_reduce(admm_handle* h, int B, int grid, const float* t_f32, const double* wnorm, double* obj_slot, cudaStream_t s);
 void launch_gather_rows(const float* src, int64_t ld, const int32_t* plan_slot, int B, int64_t n, float* dst, cudaStream_t s);
-void launch_state_out(admm_handle* h, const EpiParams& ep, int slot, double beta, float* z1, float* y1, double* z2, double* y2, cudaStream_t s);
+void launch_state_out(admm_handle* h, const EpiParams& ep, int slot, float* z1, float* y1, double* z2, double* y2, cudaStream_t s);
 int k2b_grid(const admm_handle* h, int Bact);
 int k2_choose_wj(const admm_handle* h, int Bpad);
 void launch_split_small(const float* x, int64_t count, int64_t ld, void* hi, void* lo, bool bf16, cudaStream_t s);

@@ -148,10 +148,12 @@ struct Profiler {
 void free_all(admm_handle* h) {
     void* ptrs[] = {h->d_phi, h->d_phiT, h->d_phi_t, h->d_phiT_t, h->d_csr_ptr, h->d_csrT_ptr, h->d_csr_col, h->d_csrT_col, h->d_csr_val, h->d_csrT_val, h->d_small_t, h->d_point_class, h->d_R, h->d_Sinv, h->d_s1, h->d_ghi, h->d_glo, h->d_s2, h->d_rhs,
                     h->d_vhi, h->d_vlo, h->d_partial, h->d_resid1, h->d_resid2, h->d_hinge, h->d_mask, h->d_slot_plan,
-                    h->d_utab, h->d_crtab, h->d_beta, h->d_rho, h->d_active_counts, h->d_conv_flags, h->d_res_slot,
-                    h->d_rowtmp, h->d_rowtmp2, h->d_units_k1, h->d_cta_begin_k1, h->d_mtile_slot_begin, h->d_units_k3,
-                    h->d_cta_begin_k3};
+                    h->d_utab, h->d_crtab, h->d_beta, h->d_rho, h->d_active_counts, h->d_conv_flags, h->d_bact, h->d_moves,
+                    h->d_nmoves, h->d_iters_plan, h->d_res_plan, h->d_wnorm, h->d_t_f32, h->d_obj, h->d_plan_slot, h->d_tout,
+                    h->d_qbuf, h->d_units_k1, h->d_cta_begin_k1, h->d_mtile_slot_begin, h->d_units_k3, h->d_cta_begin_k3};
     for (void* p : ptrs) if (p) cudaFree(p);
+    if (h->h_bact_ring) cudaFreeHost(h->h_bact_ring);
+    for (cudaEvent_t e : h->bact_ev) if (e) cudaEventDestroy(e);
 }
 
 EpiParams base_epi(admm_handle* h) {
@@ -172,6 +174,7 @@ EpiParams base_epi(admm_handle* h) {
     ep.s1 = h->d_s1; ep.g_hi = h->d_ghi; ep.g_lo = h->d_glo;
     ep.resid_partial = nullptr; ep.hinge_partial = h->d_hinge;
     ep.small_bf16 = h->opt.storage == ADMM_STORAGE_BF16 ? 1 : 0;
+    ep.bact_dev = nullptr;          // set by the iteration loop only: start-up, finalise and the probes act on exact slot ranges
     return ep;
 }
 
@@ -191,9 +194,11 @@ int max_pass(const admm_handle* h) {
     return (mma_passes(h) == 3 && h->opt.kernel_path == ADMM_PATH_TCGEN05) ? 96 : kMaxMmaN;
 }
 
-// one contraction pass over slots [slot0, slot0 + nact): big operand + small hi/lo rows starting at slot0
+// one contraction pass over slots [slot0, slot0 + nact): big operand + small hi/lo rows starting at slot0.
+// The four tensor maps of a (contraction, slot0, n_mma) are encoded once per batch allocation and kept (an encode costs a few
+// microseconds of host time, eight of them per iteration were a visible share of a 0.2 ms iteration).
 admm_status contract(admm_handle* h, int epi, int slot0, int nact, const float* small_hi, const float* small_lo,
-                     bool resid, float* qraw = nullptr) {
+                     bool resid, float* qraw = nullptr, bool live_from_device = false) {
     const int n_mma = (int)round_up(nact, 16);
     TcLaunch L{};
     const bool k1 = (epi == EPI_K1_PARTIAL);
@@ -202,14 +207,23 @@ admm_status contract(admm_handle* h, int epi, int slot0, int nact, const float* 
     const bool bf16 = h->opt.storage == ADMM_STORAGE_BF16;
     const int eb = bf16 ? 2 : 4, kblk = h->kblk;
     const int64_t kb_total = cdiv(big_cols, kblk), tiled_rows = cdiv(big_rows, kTileM) * kb_total * kTileM;
-    ST_TRY(tc_make_map(h, &L.map_big, k1 ? h->d_phiT_t : h->d_phi_t, tiled_rows, kblk, kblk, kBoxRows, eb));
-    ST_TRY(tc_make_map(h, &L.map_big128, k1 ? h->d_phiT_t : h->d_phi_t, tiled_rows, kblk, kblk, kTileM, eb));
+    const int kind = k1 ? 0 : 1;          // the small operand of K3 / objective / probe(1) is always the V buffer pair
+    const admm_handle::MapKey* hit = nullptr;
+    for (const auto& m : h->map_cache) if (m.kind == kind && m.slot0 == slot0 && m.n_mma == n_mma) { hit = &m; break; }
+    if (!hit) {
+        admm_handle::MapKey m{}; m.kind = kind; m.slot0 = slot0; m.n_mma = n_mma;
+        ST_TRY(tc_make_map(h, &m.big, k1 ? h->d_phiT_t : h->d_phi_t, tiled_rows, kblk, kblk, kBoxRows, eb));
+        ST_TRY(tc_make_map(h, &m.big128, k1 ? h->d_phiT_t : h->d_phi_t, tiled_rows, kblk, kblk, kTileM, eb));
+        // the small operand has Bpad rows allocated (row pitch big_ld * 4 bytes whatever the element type); rows >= nact of the
+        // box are dead columns of D
+        ST_TRY(tc_make_map(h, &m.hi, small_hi + (int64_t)slot0 * big_ld, h->Bpad - slot0, big_cols, bf16 ? 2 * big_ld : big_ld, n_mma, eb));
+        ST_TRY(tc_make_map(h, &m.lo, small_lo + (int64_t)slot0 * big_ld, h->Bpad - slot0, big_cols, bf16 ? 2 * big_ld : big_ld, n_mma, eb));
+        h->map_cache.push_back(m);
+        hit = &h->map_cache.back();
+    }
+    L.map_big = hit->big; L.map_big128 = hit->big128; L.map_small_hi = hit->hi; L.map_small_lo = hit->lo;
     L.big_kb_total = (int32_t)kb_total;
     L.kblk = kblk; L.mma_kind = bf16 ? 1 : 0;
-    // the small operand has Bpad rows allocated (row pitch big_ld * 4 bytes whatever the element type); rows >= nact of the
-    // box are dead columns of D
-    ST_TRY(tc_make_map(h, &L.map_small_hi, small_hi + (int64_t)slot0 * big_ld, h->Bpad - slot0, big_cols, bf16 ? 2 * big_ld : big_ld, n_mma, eb));
-    ST_TRY(tc_make_map(h, &L.map_small_lo, small_lo + (int64_t)slot0 * big_ld, h->Bpad - slot0, big_cols, bf16 ? 2 * big_ld : big_ld, n_mma, eb));
     L.units = k1 ? h->d_units_k1 : h->d_units_k3;
     L.cta_unit_begin = k1 ? h->d_cta_begin_k1 : h->d_cta_begin_k3;
     L.grid = k1 ? h->grid_k1 : h->grid_k3;
@@ -218,6 +232,7 @@ admm_status contract(admm_handle* h, int epi, int slot0, int nact, const float* 
     L.chunk_kb = chunk_kb(h);
     L.ep = base_epi(h);
     L.ep.slot0 = slot0; L.ep.n_slots_active = nact; L.ep.n_mma = n_mma;
+    L.ep.bact_dev = live_from_device ? h->d_bact : nullptr;
     L.ep.resid_partial = resid ? h->d_resid1 : nullptr;
     L.ep.qraw = qraw;
     return tc_launch(h, L);
@@ -239,6 +254,7 @@ void admm_default_options(admm_options* opt) {
     opt->check_every = 10;
     opt->eps_abs = 1e-6f;
     opt->compaction = 1;
+    opt->presolve = 1;
 }
 
 const char* admm_version(void) { return "paper_2509_08602_b200 0.1 sm_100a"; }
@@ -440,6 +456,8 @@ admm_status admm_setup(admm_handle** out, const float* phi, int32_t phi_on_devic
     if (o.check_every <= 0) o.check_every = 10;
     if (!(o.eps_abs > 0.f)) o.eps_abs = 1e-6f;
     if (o.storage < ADMM_STORAGE_FP32_3XTF32 || o.storage > ADMM_STORAGE_CSR) { g_setup_err = "unknown storage mode"; return ADMM_EINVAL; }
+    if (o.compaction != 1) { g_setup_err = "compaction must be 1 (masking without compaction is not offered)"; return ADMM_EINVAL; }
+    for (int r : o.reserved) if (r != 0) { g_setup_err = "admm_options.reserved must be 0"; return ADMM_EINVAL; }
     if (o.storage == ADMM_STORAGE_CSR) {
         // sparse contractions run on the plain FP32 ALUs with the orchestration of the cross-check path
         o.kernel_path = ADMM_PATH_SIMT;
@@ -470,7 +488,11 @@ admm_status admm_setup(admm_handle** out, const float* phi, int32_t phi_on_devic
 static admm_status ensure_batch_buffers(admm_handle* h, int B) {
     const int Bpad = (int)round_up(B, 16);
     if (Bpad <= h->Bpad && h->d_s1) return ADMM_OK;
+    // the epilogues address [slot][ldN] arrays with 32-bit element offsets
+    if ((int64_t)Bpad * h->ldN >= (1ll << 32)) { h->err = "B * N too large: the batch arrays must hold fewer than 2^32 elements"; return ADMM_EINVAL; }
     const bool simt = h->opt.kernel_path == ADMM_PATH_SIMT;
+    h->map_cache.clear();
+    h->Bpad = 0;
     h->k2_wj = k2_choose_wj(h, Bpad);
     ST_TRY(dev_alloc(h, &h->d_s1, (int64_t)Bpad * h->ldN));
     ST_TRY(dev_alloc(h, &h->d_ghi, (int64_t)Bpad * h->ldN));
@@ -490,11 +512,23 @@ static admm_status ensure_batch_buffers(admm_handle* h, int B) {
     ST_TRY(dev_alloc(h, &h->d_crtab, kMaxClasses * kMaxBpad));
     ST_TRY(dev_alloc(h, &h->d_beta, kMaxBpad));
     ST_TRY(dev_alloc(h, &h->d_rho, kMaxBpad));
+    ST_TRY(dev_alloc(h, &h->d_wnorm, (int64_t)kMaxBpad * kMaxClasses));
     ST_TRY(dev_alloc(h, &h->d_active_counts, (int64_t)Bpad * kMaxClasses));
     ST_TRY(dev_alloc(h, &h->d_conv_flags, Bpad));
-    ST_TRY(dev_alloc(h, &h->d_res_slot, 2 * Bpad));
-    ST_TRY(dev_alloc(h, &h->d_rowtmp, h->ldN));
-    ST_TRY(dev_alloc(h, &h->d_rowtmp2, h->ldn));
+    ST_TRY(dev_alloc(h, &h->d_bact, 1));
+    ST_TRY(dev_alloc(h, &h->d_moves, Bpad));
+    ST_TRY(dev_alloc(h, &h->d_nmoves, 1));
+    ST_TRY(dev_alloc(h, &h->d_iters_plan, Bpad));
+    ST_TRY(dev_alloc(h, &h->d_res_plan, 2 * Bpad));
+    ST_TRY(dev_alloc(h, &h->d_t_f32, (int64_t)Bpad * h->ldn));
+    ST_TRY(dev_alloc(h, &h->d_obj, kMaxBpad));
+    ST_TRY(dev_alloc(h, &h->d_plan_slot, Bpad));
+    ST_TRY(dev_alloc(h, &h->d_tout, (int64_t)Bpad * h->n));
+    if (simt) ST_TRY(dev_alloc(h, &h->d_qbuf, (int64_t)std::min(Bpad, max_pass(h)) * h->ldN));
+    if (!h->h_bact_ring) {
+        CU_TRY(h, cudaHostAlloc(reinterpret_cast<void**>(&h->h_bact_ring), 8 * sizeof(int32_t), cudaHostAllocDefault));
+        for (auto& e : h->bact_ev) CU_TRY(h, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
     h->Bpad = Bpad;
     return ADMM_OK;
 }
@@ -504,24 +538,43 @@ struct SlotTables {
     std::vector<float> utab, crtab;         // [kMaxClasses][kMaxBpad]
     std::vector<double> beta, rho, wnorm;   // [kMaxBpad], [kMaxBpad][kMaxClasses]
 };
-admm_status upload_tables(admm_handle* h, const SlotTables& T, double* d_wnorm) {
+admm_status upload_tables(admm_handle* h, const SlotTables& T) {
     cudaStream_t st = h->stream;
     CU_TRY(h, cudaMemcpyAsync(h->d_utab, T.utab.data(), T.utab.size() * 4, cudaMemcpyHostToDevice, st));
     CU_TRY(h, cudaMemcpyAsync(h->d_crtab, T.crtab.data(), T.crtab.size() * 4, cudaMemcpyHostToDevice, st));
     CU_TRY(h, cudaMemcpyAsync(h->d_beta, T.beta.data(), T.beta.size() * 8, cudaMemcpyHostToDevice, st));
     CU_TRY(h, cudaMemcpyAsync(h->d_rho, T.rho.data(), T.rho.size() * 8, cudaMemcpyHostToDevice, st));
     CU_TRY(h, cudaMemcpyAsync(h->d_slot_plan, h->slot_plan.data(), h->slot_plan.size() * 4, cudaMemcpyHostToDevice, st));
-    if (d_wnorm) CU_TRY(h, cudaMemcpyAsync(d_wnorm, T.wnorm.data(), T.wnorm.size() * 8, cudaMemcpyHostToDevice, st));
+    CU_TRY(h, cudaMemcpyAsync(h->d_wnorm, T.wnorm.data(), T.wnorm.size() * 8, cudaMemcpyHostToDevice, st));
     return ADMM_OK;
 }
-template <typename T>
-admm_status swap_rows(admm_handle* h, T* base, int64_t ld, int a, int b, T* tmp) {
-    cudaStream_t st = h->stream;
-    CU_TRY(h, cudaMemcpyAsync(tmp, base + (int64_t)a * ld, (size_t)ld * sizeof(T), cudaMemcpyDeviceToDevice, st));
-    CU_TRY(h, cudaMemcpyAsync(base + (int64_t)a * ld, base + (int64_t)b * ld, (size_t)ld * sizeof(T), cudaMemcpyDeviceToDevice, st));
-    CU_TRY(h, cudaMemcpyAsync(base + (int64_t)b * ld, tmp, (size_t)ld * sizeof(T), cudaMemcpyDeviceToDevice, st));
-    return ADMM_OK;
-}
+// The live count after each check travels to the host through a small ring of pinned words + events.  The host never waits for the
+// check it has just enqueued: it waits for the one before, so a whole check interval of work is always queued behind the GPU and
+// the launch sizes (n_mma, grids) follow the device's live count with a lag of at most one interval.
+struct LiveCount {
+    admm_handle* h; int head = 0, tail = 0;        // ring entries [tail, head) are in flight
+    admm_status push() {
+        const int e = head % 8;
+        CU_TRY(h, cudaMemcpyAsync(h->h_bact_ring + e, h->d_bact, 4, cudaMemcpyDeviceToHost, h->stream));
+        CU_TRY(h, cudaEventRecord(h->bact_ev[e], h->stream));
+        ++head;
+        return ADMM_OK;
+    }
+    // waits until at most `keep` copies are still in flight; returns the newest value that has arrived (or `cur`)
+    admm_status drain(int keep, int* cur) {
+        while (head - tail > keep) {
+            const int e = tail % 8;
+            CU_TRY(h, cudaEventSynchronize(h->bact_ev[e]));
+            *cur = std::min(*cur, (int)h->h_bact_ring[e]);
+            ++tail;
+        }
+        while (head > tail && cudaEventQuery(h->bact_ev[tail % 8]) == cudaSuccess) {
+            *cur = std::min(*cur, (int)h->h_bact_ring[tail % 8]);
+            ++tail;
+        }
+        return ADMM_OK;
+    }
+};
 }  // namespace
 
 extern "C" {
@@ -542,7 +595,7 @@ admm_status admm_solve_batch(admm_handle* h, int32_t B, const float* weights, co
     CU_TRY(h, cudaSetDevice(h->opt.device));
     cudaStream_t st = h->stream;
     const double wall0 = now_ms();
-    h->launch_count = 0; h->ktimes = KernelTimes{}; h->plan_iters = 0; h->solved = false;
+    h->launch_count = 0; h->ktimes = KernelTimes{}; h->plan_iters = 0; h->solved = false; h->presolved = 0;
     ST_TRY(ensure_batch_buffers(h, B));
     h->B = B;
     const bool simt = h->opt.kernel_path == ADMM_PATH_SIMT;
@@ -553,8 +606,10 @@ admm_status admm_solve_batch(admm_handle* h, int32_t B, const float* weights, co
     h->mask_words = cdiv(h->N, 32);
     h->has_mask = row_mask != nullptr;
     if (row_mask) {
-        if (h->d_mask) { cudaFree(h->d_mask); h->d_mask = nullptr; }
-        ST_TRY(dev_alloc(h, &h->d_mask, (int64_t)B * h->mask_words));
+        if ((int64_t)B * h->mask_words > h->mask_capacity) {
+            ST_TRY(dev_alloc(h, &h->d_mask, (int64_t)B * h->mask_words));
+            h->mask_capacity = (int64_t)B * h->mask_words;
+        }
         CU_TRY(h, cudaMemcpyAsync(h->d_mask, row_mask, (size_t)B * h->mask_words * 4,
                                   is_device_ptr(row_mask) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
     }
@@ -568,30 +623,31 @@ admm_status admm_solve_batch(admm_handle* h, int32_t B, const float* weights, co
     T.utab.assign((size_t)kMaxClasses * kMaxBpad, 0.f); T.crtab.assign((size_t)kMaxClasses * kMaxBpad, 0.f);
     T.beta.assign(kMaxBpad, 0.0); T.rho.assign(kMaxBpad, 1.0); T.wnorm.assign((size_t)kMaxBpad * kMaxClasses, 0.0);
     h->slot_plan.assign(h->Bpad, 0); h->plan_slot.assign(B, 0); h->iters.assign(B, 0);
-    h->h_weights.assign(weights, weights + (size_t)B * W);
-    std::vector<float> res_plan((size_t)2 * B, 0.f);
     int64_t n_min_class = h->class_count[0];
     for (int k = 1; k < K; ++k) n_min_class = std::min(n_min_class, h->class_count[k]);
+    bool box_optimum_finite = true;           // presolve needs a finite box optimum: no hard class with c < 0
+    for (int k = 0; k < K; ++k) if (h->classes[k].hard && h->classes[k].sense > 0) box_optimum_finite = false;
     for (int p = 0; p < B; ++p) {
         const double beta = weights[(size_t)p * W + K];
-        // default: (kappa / N_min) sqrt(beta0 / max(beta, beta0/64)), kappa = 1, beta0 = 0.05 (reading R8)
-        const double r = rho ? (double)rho[p] : (1.0 / (double)n_min_class) * std::sqrt(0.05 / std::max(beta, 0.05 / 64.0));
+        // default: (kappa / N_min) sqrt(beta0 / max(beta, beta0/floor)), kappa = 1, beta0 = 0.05 (reading R8)
+        const double r = rho ? (double)rho[p] : (1.0 / (double)n_min_class) * std::sqrt(0.05 / std::max(beta, 0.05 / kRhoFloorDiv));
         T.beta[p] = beta; T.rho[p] = r;
         for (int k = 0; k < K; ++k) {
             const double Nk = (double)h->class_count[k], Nkp = (double)counts[(size_t)p * kMaxClasses + k];
             const double wk = weights[(size_t)p * W + k], thr = h->classes[k].threshold, sense = h->classes[k].sense;
-            // u_hat = u / D = (w thr / N_kp) * N_k ;  c_hat / rho = (-sense / N_k) / rho
-            T.utab[(size_t)k * kMaxBpad + p] = (float)(Nkp > 0 ? wk * thr * Nk / Nkp : 0.0);
+            // u_hat = u / D = (w thr / N_kp) * N_k ;  c_hat / rho = (-sense / N_k) / rho ;  hard class: u = infinity (Eq. 15)
+            float uh = (float)(Nkp > 0 ? wk * thr * Nk / Nkp : 0.0);
+            if (h->classes[k].hard) uh = Nkp > 0 ? INFINITY : 0.f;
+            T.utab[(size_t)k * kMaxBpad + p] = uh;
             T.crtab[(size_t)k * kMaxBpad + p] = (float)((-sense / Nk) / r);
-            T.wnorm[(size_t)p * kMaxClasses + k] = Nkp > 0 ? wk / Nkp : 0.0;
+            T.wnorm[(size_t)p * kMaxClasses + k] = (Nkp > 0 && !h->classes[k].hard) ? wk / Nkp : 0.0;
         }
         h->slot_plan[p] = p; h->plan_slot[p] = p;
     }
-    h->h_beta = T.beta; h->h_rho = T.rho;
-    double* d_wnorm = nullptr;
-    ST_TRY(dev_alloc(h, &d_wnorm, (int64_t)kMaxBpad * kMaxClasses));
-    struct Guard { double* p; ~Guard() { if (p) cudaFree(p); } } guard{d_wnorm};
-    ST_TRY(upload_tables(h, T, d_wnorm));
+    ST_TRY(upload_tables(h, T));
+    const int32_t B32 = B;
+    CU_TRY(h, cudaMemcpyAsync(h->d_bact, &B32, 4, cudaMemcpyHostToDevice, st));
+    launch_init_plan_records(h, B, st);
 
     // ---- zero start (R6) and the first K1 operand
     CU_TRY(h, cudaMemsetAsync(h->d_s1, 0, (size_t)h->Bpad * h->ldN * 4, st));
@@ -600,13 +656,7 @@ admm_status admm_solve_batch(admm_handle* h, int32_t B, const float* weights, co
     CU_TRY(h, cudaMemsetAsync(h->d_s2, 0, (size_t)h->Bpad * h->ldn * 8, st));
     CU_TRY(h, cudaMemsetAsync(h->d_vhi, 0, (size_t)h->Bpad * h->ldn * 4, st));
     CU_TRY(h, cudaMemsetAsync(h->d_vlo, 0, (size_t)h->Bpad * h->ldn * 4, st));
-    {
-        EpiParams ep = base_epi(h); ep.slot0 = 0; ep.n_slots_active = B;
-        launch_emit_g(ep, B, st); h->launch_count++;
-    }
-    float* qbuf = nullptr;     // SIMT path only: Q [chunk][ldN]
-    if (simt) ST_TRY(dev_alloc(h, &qbuf, (int64_t)std::min(h->Bpad, max_pass(h)) * h->ldN));
-    struct Guard2 { float* p; ~Guard2() { if (p) cudaFree(p); } } guard2{qbuf};
+    float* qbuf = h->d_qbuf;     // SIMT path only: Q [pass][ldN]
 
     Profiler prof; prof.on = h->opt.profile_kernels != 0;
     cudaEvent_t ev0, ev1, ev2;
@@ -614,21 +664,42 @@ admm_status admm_solve_batch(admm_handle* h, int32_t B, const float* weights, co
     struct EvGuard { cudaEvent_t a, b, c; ~EvGuard() { cudaEventDestroy(a); cudaEventDestroy(b); cudaEventDestroy(c); } } evg{ev0, ev1, ev2};
     cudaEventRecord(ev0, st);
 
-    int Bact = B;
-    std::vector<int32_t> flags(h->Bpad);
-    std::vector<float> res_slot((size_t)2 * h->Bpad);
+    int Bact = B;                       // the HOST's upper bound on the live count; the device's own is *d_bact
+    LiveCount live{h};
+    EpiParams ep0 = base_epi(h); ep0.slot0 = 0; ep0.n_slots_active = B;
+
+    // ---- presolve (deviation D1): plans whose box optimum is feasible are solved in closed form (t* = 0)
+    if (fixed_iters == 0 && h->opt.presolve && box_optimum_finite) {
+        launch_presolve_state(ep0, B, st);
+        launch_emit_g(ep0, B, st);
+        for (int s0 = 0; s0 < B; s0 += max_pass(h)) {
+            const int nact = std::min(max_pass(h), B - s0);
+            const int n_mma = (int)round_up(nact, 16);
+            if (simt) launch_simt_k1(h, s0, nact, n_mma, h->grid_k1, st);
+            else ST_TRY(contract(h, EPI_K1_PARTIAL, s0, nact, h->d_ghi, h->d_glo, false));
+            launch_presolve_test(h, s0, nact, n_mma, 1e-5, st);
+        }
+        launch_presolve_reset(h, B, st);
+        h->launch_count += 4;
+        launch_compaction(h, Bact, st);
+        ST_TRY(live.push());
+        ST_TRY(live.drain(0, &Bact));
+        h->presolved = B - Bact;
+    }
+    if (Bact > 0) { ep0.n_slots_active = Bact; launch_emit_g(ep0, Bact, st); h->launch_count++; }
+
     const int grid1 = simt ? (int)cdiv(h->N, 128) : h->grid_k3;
     int it = 0;
     while (it < total_iters && Bact > 0) {
         ++it;
         const bool check = (fixed_iters > 0) ? (it == total_iters) : (it % check_every == 0 || it == total_iters);
-        // ---- K1 + K2a per chunk of <= 256 slots: rhs = R o (Phi^T G) - (2 z2 - s2)
+        // ---- K1 + K2a per pass of plans: rhs = R o (Phi^T G) - (2 z2 - s2)
         for (int s0 = 0; s0 < Bact; s0 += max_pass(h)) {
             const int nact = std::min(max_pass(h), Bact - s0);
             const int n_mma = (int)round_up(nact, 16);
             prof.begin(h, 0);
             if (simt) launch_simt_k1(h, s0, nact, n_mma, h->grid_k1, st);
-            else ST_TRY(contract(h, EPI_K1_PARTIAL, s0, nact, h->d_ghi, h->d_glo, false));
+            else ST_TRY(contract(h, EPI_K1_PARTIAL, s0, nact, h->d_ghi, h->d_glo, false, nullptr, true));
             prof.end(h);
             prof.begin(h, 1);
             launch_k2a(h, s0, nact, n_mma, st);
@@ -645,66 +716,32 @@ admm_status admm_solve_batch(admm_handle* h, int32_t B, const float* weights, co
             if (simt) {
                 EpiParams ep = base_epi(h);
                 ep.slot0 = s0; ep.n_slots_active = nact; ep.n_mma = (int)round_up(nact, 16);
+                ep.bact_dev = h->d_bact;
                 ep.resid_partial = check ? h->d_resid1 : nullptr;
                 launch_simt_k3(h, ep, EPI_K3_STATE, h->d_vhi + (int64_t)s0 * h->ldn, h->d_vlo + (int64_t)s0 * h->ldn, qbuf, st);
             } else {
-                ST_TRY(contract(h, EPI_K3_STATE, s0, nact, h->d_vhi, h->d_vlo, check));
+                ST_TRY(contract(h, EPI_K3_STATE, s0, nact, h->d_vhi, h->d_vlo, check, nullptr, true));
             }
             prof.end(h);
         }
         if (!check) continue;
-        // ---- H5: stopping rule, freeze + compaction
+        // ---- H5: stopping rule on the device, then (tolerance mode) compaction on the device
         prof.begin(h, 3);
-        launch_convergence(h, Bact, grid1, k2b_grid(h, Bact), fixed_iters > 0 ? 0.f : tol, h->opt.eps_abs, st);
+        launch_convergence(h, Bact, grid1, k2b_grid(h, Bact), fixed_iters > 0 ? 0.f : tol, h->opt.eps_abs, it, st);
+        if (fixed_iters == 0) launch_compaction(h, Bact, st);
         prof.end(h);
-        CU_TRY(h, cudaMemcpyAsync(flags.data(), h->d_conv_flags, (size_t)Bact * 4, cudaMemcpyDeviceToHost, st));
-        CU_TRY(h, cudaMemcpyAsync(res_slot.data(), h->d_res_slot, (size_t)Bact * 8, cudaMemcpyDeviceToHost, st));
-        CU_TRY(h, cudaStreamSynchronize(st));
-        prof.harvest(h);
-        for (int s = 0; s < Bact; ++s) {
-            const int p = h->slot_plan[s];
-            h->iters[p] = it;
-            res_plan[2 * p] = res_slot[2 * s]; res_plan[2 * p + 1] = res_slot[2 * s + 1];
+        if (fixed_iters == 0) {
+            ST_TRY(live.push());
+            ST_TRY(live.drain(1, &Bact));           // wait for the PREVIOUS check only: the GPU always has an interval queued
         }
-        if (fixed_iters > 0) continue;
-        bool changed = false;
-        for (int s = Bact - 1; s >= 0; --s) {
-            if (!flags[s]) continue;
-            if (!h->opt.compaction) continue;
-            const int last = Bact - 1;
-            if (s != last) {
-                ST_TRY(swap_rows(h, h->d_s1, h->ldN, s, last, h->d_rowtmp));
-                ST_TRY(swap_rows(h, h->d_ghi, h->ldN, s, last, h->d_rowtmp));
-                ST_TRY(swap_rows(h, h->d_glo, h->ldN, s, last, h->d_rowtmp));
-                ST_TRY(swap_rows(h, h->d_s2, h->ldn, s, last, h->d_rowtmp2));
-                for (int k = 0; k < kMaxClasses; ++k) {
-                    std::swap(T.utab[(size_t)k * kMaxBpad + s], T.utab[(size_t)k * kMaxBpad + last]);
-                    std::swap(T.crtab[(size_t)k * kMaxBpad + s], T.crtab[(size_t)k * kMaxBpad + last]);
-                    std::swap(T.wnorm[(size_t)s * kMaxClasses + k], T.wnorm[(size_t)last * kMaxClasses + k]);
-                }
-                std::swap(T.beta[s], T.beta[last]); std::swap(T.rho[s], T.rho[last]);
-                std::swap(h->slot_plan[s], h->slot_plan[last]);
-                h->plan_slot[h->slot_plan[s]] = s; h->plan_slot[h->slot_plan[last]] = last;
-            }
-            --Bact; changed = true;
-        }
-        if (changed) { ST_TRY(upload_tables(h, T, d_wnorm)); h->launch_count += 0; }
-        if (!h->opt.compaction) {
-            bool all = true;
-            for (int s = 0; s < Bact; ++s) all = all && flags[s];
-            if (all) break;
-        }
+        if (cudaGetLastError() != cudaSuccess) { h->err = "a hot-path kernel failed to launch"; return ADMM_ECUDA; }
     }
-    h->h_beta = T.beta; h->h_rho = T.rho;
+    ST_TRY(live.drain(0, &Bact));
     cudaEventRecord(ev1, st);
 
-    // ---- H6: t = rho R y2, objective P(t) through one more Phi contraction
+    // ---- H6: t = rho R y2, objective P(t) through one more Phi contraction (all B slots, frozen ones included)
     float *t_hi = h->d_vhi, *t_lo = h->d_vlo;          // v operands are dead now: reuse as the T operand
-    float* t_f32 = nullptr; double* d_obj = nullptr; float* d_tout = nullptr; int32_t* d_plan_slot = nullptr;
-    ST_TRY(dev_alloc(h, &t_f32, (int64_t)h->Bpad * h->ldn));
-    struct Guard3 { void* a; void* b; void* c; void* d; ~Guard3() { cudaFree(a); if (b) cudaFree(b); if (c) cudaFree(c); if (d) cudaFree(d); } } guard3{t_f32, nullptr, nullptr, nullptr};
-    ST_TRY(dev_alloc(h, &d_obj, kMaxBpad)); guard3.b = d_obj;
-    ST_TRY(dev_alloc(h, &d_plan_slot, B)); guard3.d = d_plan_slot;
+    float* t_f32 = h->d_t_f32;
     launch_make_t(h, B, t_hi, t_lo, t_f32, st);
     for (int s0 = 0; s0 < B; s0 += max_pass(h)) {
         const int nact = std::min(max_pass(h), B - s0);
@@ -716,26 +753,33 @@ admm_status admm_solve_batch(admm_handle* h, int32_t B, const float* weights, co
             ST_TRY(contract(h, EPI_OBJECTIVE, s0, nact, t_hi, t_lo, false));
         }
     }
-    launch_objective_reduce(h, B, grid1, t_f32, d_wnorm, d_obj, st);
+    launch_objective_reduce(h, B, grid1, t_f32, h->d_wnorm, h->d_obj, st);
     cudaEventRecord(ev2, st);
 
-    // ---- outputs, in plan order
-    CU_TRY(h, cudaMemcpyAsync(d_plan_slot, h->plan_slot.data(), (size_t)B * 4, cudaMemcpyHostToDevice, st));
-    if (t_out) {
-        if (is_device_ptr(t_out)) {
-            launch_gather_rows(t_f32, h->ldn, d_plan_slot, B, h->n, t_out, st);
-        } else {
-            ST_TRY(dev_alloc(h, &d_tout, (int64_t)B * h->n)); guard3.c = d_tout;
-            launch_gather_rows(t_f32, h->ldn, d_plan_slot, B, h->n, d_tout, st);
-            CU_TRY(h, cudaMemcpyAsync(t_out, d_tout, (size_t)B * h->n * 4, cudaMemcpyDeviceToHost, st));
-        }
-    }
+    // ---- read back what the host needs; nothing of the caller's is written until everything has succeeded
     std::vector<double> obj_slot(B);
-    CU_TRY(h, cudaMemcpyAsync(obj_slot.data(), d_obj, (size_t)B * 8, cudaMemcpyDeviceToHost, st));
+    std::vector<float> res_plan((size_t)2 * B);
+    CU_TRY(h, cudaMemcpyAsync(h->slot_plan.data(), h->d_slot_plan, (size_t)B * 4, cudaMemcpyDeviceToHost, st));
+    CU_TRY(h, cudaMemcpyAsync(obj_slot.data(), h->d_obj, (size_t)B * 8, cudaMemcpyDeviceToHost, st));
+    CU_TRY(h, cudaMemcpyAsync(h->iters.data(), h->d_iters_plan, (size_t)B * 4, cudaMemcpyDeviceToHost, st));
+    CU_TRY(h, cudaMemcpyAsync(res_plan.data(), h->d_res_plan, (size_t)B * 8, cudaMemcpyDeviceToHost, st));
     CU_TRY(h, cudaStreamSynchronize(st));
+    if (cudaGetLastError() != cudaSuccess) { h->err = "a hot-path kernel failed"; return ADMM_ECUDA; }
     prof.harvest(h);
+    for (int s = 0; s < B; ++s) h->plan_slot[h->slot_plan[s]] = s;
     std::vector<double> obj_plan(B);
     for (int p = 0; p < B; ++p) obj_plan[p] = obj_slot[h->plan_slot[p]];
+    // ---- outputs, in plan order
+    if (t_out) {
+        CU_TRY(h, cudaMemcpyAsync(h->d_plan_slot, h->plan_slot.data(), (size_t)B * 4, cudaMemcpyHostToDevice, st));
+        if (is_device_ptr(t_out)) {
+            launch_gather_rows(t_f32, h->ldn, h->d_plan_slot, B, h->n, t_out, st);
+        } else {
+            launch_gather_rows(t_f32, h->ldn, h->d_plan_slot, B, h->n, h->d_tout, st);
+            CU_TRY(h, cudaMemcpyAsync(t_out, h->d_tout, (size_t)B * h->n * 4, cudaMemcpyDeviceToHost, st));
+        }
+        CU_TRY(h, cudaStreamSynchronize(st));
+    }
     auto put = [&](void* dst, const void* src, size_t bytes) -> cudaError_t {
         if (!dst) return cudaSuccess;
         if (is_device_ptr(dst)) return cudaMemcpy(dst, src, bytes, cudaMemcpyHostToDevice);
@@ -814,7 +858,7 @@ admm_status admm_get_state(admm_handle* h, int32_t plan, float* z1, float* y1, d
     ST_TRY(stage(&dz1, z1, h->N, 0)); ST_TRY(stage(&dy1, y1, h->N, 1));
     ST_TRY(stage(&dz2, z2, h->n, 2)); ST_TRY(stage(&dy2, y2, h->n, 3));
     EpiParams ep = base_epi(h);
-    launch_state_out(h, ep, slot, h->h_beta[slot], dz1, dy1, dz2, dy2, st);
+    launch_state_out(h, ep, slot, dz1, dy1, dz2, dy2, st);
     if (g.p[0]) CU_TRY(h, cudaMemcpyAsync(z1, dz1, (size_t)h->N * 4, cudaMemcpyDeviceToHost, st));
     if (g.p[1]) CU_TRY(h, cudaMemcpyAsync(y1, dy1, (size_t)h->N * 4, cudaMemcpyDeviceToHost, st));
     if (g.p[2]) CU_TRY(h, cudaMemcpyAsync(z2, dz2, (size_t)h->n * 8, cudaMemcpyDeviceToHost, st));

@@ -4,18 +4,17 @@
 //   K3  Q   = Phi   . V      "A^T v"  of Eq. (7), PAPER.md:93   big operand Phi  [N][n], small operand V  [B][n]
 //   OBJ dose= Phi   . T      primal objective, PAPER.md:183     (K3's mainloop, another epilogue)
 //
-// One kernel serves all three.  D[128 rows of the big operand][plans] accumulates in TMEM (fp32).
-// Both operands are K-major fp32 tiles of 32 elements (one 128-byte swizzle row) staged by TMA.
-// "fp32 path" = 3xTF32: the small operand arrives pre-split (hi on the tf32 grid, lo = x - hi, both written
-// by the producing epilogue); the big operand (Phi) is read ONCE from HBM as fp32 and split on chip by four
-// converter warps (hi = bits above the tf32 cut, lo = x - hi, exact), then
-//     D += Phi_lo.G_hi ; D += Phi_hi.G_lo ; D += Phi_hi.G_hi          (small terms first)
-// With mma_passes == 2 the big operand is already on the tf32 grid (ADMM_STORAGE_FP32_TF32), no converter.
+// D[128 rows of the big operand][plans] accumulates in TMEM (fp32).  Both operands are K-major tiles of 128-byte rows
+// (32 fp32 / 64 bf16 elements, one swizzle row) staged by TMA; the big operand is stored tile-major in HBM.
+// "fp32 path" = 3xTF32: the small operand arrives pre-split (hi on the tf32 grid, lo = x - hi, both written by the producing
+// epilogue); the big operand (Phi) is read ONCE from HBM as fp32 and split on chip.
 //
-// Warp roles (320 threads, 1 CTA / SM, persistent over a host-built unit list):
-//   warp 0      TMA producer (one lane)           warp 1      UMMA issuer (one lane) + TMEM alloc/dealloc
-//   warps 2-5   converter (hi/lo split in smem)    warps 6-9   epilogue (TMEM -> registers -> global)
-// Pipelines: smem ring full[s] -> (conv[s]) -> empty[s]; TMEM double buffer tmem_full[a] / tmem_empty[a].
+// Three kernels, chosen by tc_launch():
+//   admm_contract_f32_kernel   passes of <= 96 plans, every storage mode (3xTF32: converter -> TMEM A ring, TS-form MMAs,
+//                              drained accumulation, staged epilogue; tf32 / bf16 storage: A straight from shared memory)
+//   admm_contract_wide_kernel  3xTF32 passes of 97..224 plans: hi/lo tiles in shared memory, SS-form MMAs, drained
+//                              accumulation, epilogue from the drain warps' registers
+//   admm_contract_kernel       tf32 / bf16 storage, passes of 97..256 plans: undrained accumulation, epilogue from TMEM
 #include <cstdio>
 #include <cstring>
 #include "admm_internal.h"
@@ -27,31 +26,25 @@ namespace {
 constexpr int kTileBytes = kTileM * kBlockK * 4;       // 16 KB: 128 rows x 128 B
 constexpr int kBoxBytes = kBoxRows * kBlockK * 4;      // 4 KB
 constexpr int kMaxStages = 8;
-constexpr int kAccCols = 256;                          // TMEM columns per accumulator stage (DRAIN = false)
-constexpr int kDrainCols = 128;                        // DRAIN: 2 main + 2 correction accumulators of 128 columns
+constexpr int kAccCols = 256;                          // TMEM columns per accumulator stage of admm_contract_kernel
 constexpr int kSmemLimit = 227 * 1024;
 
 struct Ctrl {
     uint64_t full[kMaxStages];
-    uint64_t conv[kMaxStages];
     uint64_t empty[kMaxStages];
     uint64_t tmem_full[2];
     uint64_t tmem_empty[2];
-    uint64_t small_full[2];     // DRAIN: accumulator of the correction terms, one per unit
-    uint64_t small_empty[2];
     uint32_t tmem_base;
     uint32_t pad;
 };
 
-__host__ __device__ inline int stage_bytes(int mma_passes, int n_mma) {
-    return kTileBytes * (mma_passes == 3 ? 2 : 1) + 2 * n_mma * kBlockK * 4;
-}
-__host__ __device__ inline int acc_bytes(int n_mma) { return 8 * n_mma * 8 * 4; }   // [8 warps][n_mma][8] floats
+__host__ __device__ inline int stage_bytes(int n_mma) { return kTileBytes + 2 * n_mma * kBlockK * 4; }
+__host__ __device__ inline int acc_bytes(int n_mma) { return 4 * n_mma * 8 * 4; }   // [4 warps][n_mma][8] floats
 
 // Everything one epilogue thread needs to process columns (plans) of its row.
 struct EpiCtx {
     bool valid; int lrow; int64_t row; int cls; float a_k, sense, thr; bool resid; int64_t mword; int lane;
-    float* wacc; int slot;
+    float* wacc; int slot; int n_act;
 };
 
 // 16 consecutive columns c0..c0+15 of this thread's row: q[jj] = accumulator of plan (slot0 + c0 + jj).
@@ -59,7 +52,7 @@ struct EpiCtx {
 // the stores are predicated) -- see epilogue_unit_t for why.
 __device__ __forceinline__ void epi_cols16(const TcLaunch& L, const EpiCtx& cx, int c0, const float (&q)[16]) {
     const EpiParams& ep = L.ep;
-    const int n_act = ep.n_slots_active;
+    const int n_act = cx.n_act;
     const int epi = L.epi;
     if (epi == EPI_K1_PARTIAL) {
         float* dst = ep.partial + ((int64_t)cx.slot * ep.n_mma) * kTileM + cx.lrow;
@@ -127,21 +120,22 @@ __device__ __forceinline__ void epi_cols16(const TcLaunch& L, const EpiCtx& cx, 
     }
 }
 
-// DRAIN = true  (fp32 path): the TMEM accumulator is emptied every L.chunk_kb k-blocks into fp32 register
-//   master sums by 8 epilogue warps (two per TMEM lane group, half of the columns each).  tcgen05.mma
-//   accumulates with round-toward-zero (measured: bias -2^-25 per MMA, linear in K, coherent over
-//   iterations); summing short chunks with round-to-nearest FADDs removes that bias.  n_mma <= 128.
-// DRAIN = false: one chunk per unit, 4 epilogue warps read the finished accumulator once.  n_mma <= 256.
-template <bool DRAIN>
-__global__ void __launch_bounds__(DRAIN ? 448 : 320, 1) admm_contract_kernel(const __grid_constant__ TcLaunch L) {
-    constexpr int kThreads = DRAIN ? 448 : 320;
-    constexpr int kEpiWarps = DRAIN ? 8 : 4;
+// tf32 / bf16 storage, passes of 97..256 plans (B = 441 in two passes).  The big operand is exact in the operand format, so the
+// A tile goes straight from shared memory into the MMAs; the plan operand is a hi/lo pair: two MMAs per 32-byte k-step into ONE
+// accumulator (lo first).  One accumulation per unit (no drain: the reduced-storage modes have a 1e-2 budget), two TMEM accumulator
+// stages of 256 columns so the 4 epilogue warps read tile i while the MMAs of tile i+1 run.
+// Warp roles (320 threads, 1 CTA / SM, persistent over a host-built unit list):
+//   warp 0  TMA producer (one lane)      warp 1  UMMA issuer (one lane) + TMEM alloc/dealloc      warps 6-9  epilogue
+__global__ void __launch_bounds__(320, 1) admm_contract_kernel(const __grid_constant__ TcLaunch L) {
+    constexpr int kThreads = 320;
+    constexpr int kEpiWarps = 4;
     extern __shared__ __align__(1024) uint8_t smem[];
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
     const int n_mma = L.ep.n_mma;
-    const int passes = L.mma_passes;
-    const int sbytes = stage_bytes(passes, n_mma);
+    const int n_act = eff_nact(L.ep);
+    if (n_act <= 0) return;                               // the whole pass froze since the host sized this launch
+    const int sbytes = stage_bytes(n_mma);
     // carve: [stages x stage][acc][ctrl]
     int n_stages = (kSmemLimit - 1024 - (int)sizeof(Ctrl) - acc_bytes(n_mma)) / sbytes;
     if (n_stages > kMaxStages) n_stages = kMaxStages;
@@ -151,19 +145,15 @@ __global__ void __launch_bounds__(DRAIN ? 448 : 320, 1) admm_contract_kernel(con
 
     const int unit_begin = L.cta_unit_begin[blockIdx.x];
     const int unit_end = L.cta_unit_begin[blockIdx.x + 1];
-    const int chunk_kb = L.chunk_kb;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < n_stages; ++s) {
             tc::mbar_init(&ctrl->full[s], 1);
-            tc::mbar_init(&ctrl->conv[s], 128);
             tc::mbar_init(&ctrl->empty[s], 1);
         }
         for (int a = 0; a < 2; ++a) {
             tc::mbar_init(&ctrl->tmem_full[a], 1);
             tc::mbar_init(&ctrl->tmem_empty[a], kEpiWarps * 32);
-            tc::mbar_init(&ctrl->small_full[a], 1);
-            tc::mbar_init(&ctrl->small_empty[a], kEpiWarps * 32);
         }
         tc::fence_barrier_init();
         tc::tma_prefetch_desc(&L.map_big);
@@ -177,9 +167,8 @@ __global__ void __launch_bounds__(DRAIN ? 448 : 320, 1) admm_contract_kernel(con
     tc::tcgen05_fence_after();
     const uint32_t tmem_base = ctrl->tmem_base;
 
-    auto stage_a_raw = [&](int s) { return stage_base + s * sbytes; };
-    auto stage_a_lo = [&](int s) { return stage_base + s * sbytes + kTileBytes; };
-    auto stage_b_hi = [&](int s) { return stage_base + s * sbytes + kTileBytes * (passes == 3 ? 2 : 1); };
+    auto stage_a = [&](int s) { return stage_base + s * sbytes; };
+    auto stage_b_hi = [&](int s) { return stage_base + s * sbytes + kTileBytes; };
     auto stage_b_lo = [&](int s) { return stage_b_hi(s) + n_mma * kBlockK * 4; };
 
     if (warp == 0) {
@@ -196,7 +185,7 @@ __global__ void __launch_bounds__(DRAIN ? 448 : 320, 1) admm_contract_kernel(con
                     const int k0 = (un.kb0 + kb) * L.kblk;
                     const int trow = ((un.row0 >> 7) * L.big_kb_total + un.kb0 + kb) * kTileM;     // tile-major big operand
                     for (int b = 0; b < nbox; ++b)
-                        tc::tma_load_2d(stage_a_raw(s) + b * kBoxBytes, &L.map_big, &ctrl->full[s], 0,
+                        tc::tma_load_2d(stage_a(s) + b * kBoxBytes, &L.map_big, &ctrl->full[s], 0,
                                         trow + b * kBoxRows, tc::kEvictFirst);
                     tc::tma_load_2d(stage_b_hi(s), &L.map_small_hi, &ctrl->full[s], k0, 0, tc::kEvictLast);
                     tc::tma_load_2d(stage_b_lo(s), &L.map_small_lo, &ctrl->full[s], k0, 0, tc::kEvictLast);
@@ -211,110 +200,47 @@ __global__ void __launch_bounds__(DRAIN ? 448 : 320, 1) admm_contract_kernel(con
             const uint32_t idesc = tc::umma_idesc(bf16 ? 1u : 2u, kTileM, (uint32_t)n_mma);
             int s = 0; uint32_t ph = 0;
             int a = 0; uint32_t aph = 0;
-            int b = 0; uint32_t bph = 0;
             for (int u = unit_begin; u < unit_end; ++u) {
                 const TcUnit un = L.units[u];
-                const int ck = DRAIN ? chunk_kb : un.kb_count;
-                // DRAIN: correction terms (lo.hi + hi.lo) accumulate over the whole unit in their own accumulator
-                const uint32_t d_small = tmem_base + 2 * kDrainCols + b * kDrainCols;
-                if (DRAIN) {
-                    tc::mbar_wait(&ctrl->small_empty[b], bph ^ 1);
-                    tc::tcgen05_fence_after();
-                }
-                for (int kb0 = 0; kb0 < un.kb_count; kb0 += ck) {
-                    const int nkb = min(ck, un.kb_count - kb0);
-                    tc::mbar_wait(&ctrl->tmem_empty[a], aph ^ 1);
-                    tc::tcgen05_fence_after();
-                    const uint32_t d_tmem = tmem_base + a * (DRAIN ? kDrainCols : kAccCols);
-                    for (int kb = 0; kb < nkb; ++kb) {
-                        tc::mbar_wait(passes == 3 ? &ctrl->conv[s] : &ctrl->full[s], ph);
-                        tc::tcgen05_fence_after();
-                        const uint64_t a_raw = tc::umma_desc_k_sw128(tc::smem_u32(stage_a_raw(s)));
-                        const uint64_t a_lo = tc::umma_desc_k_sw128(tc::smem_u32(stage_a_lo(s)));
-                        const uint64_t b_hi = tc::umma_desc_k_sw128(tc::smem_u32(stage_b_hi(s)));
-                        const uint64_t b_lo = tc::umma_desc_k_sw128(tc::smem_u32(stage_b_lo(s)));
-#pragma unroll
-                        for (int k = 0; k < kBlockK / 8; ++k) {
-                            const uint64_t koff = (uint64_t)((k * 8 * 4) >> 4);   // 32 bytes per tf32 k-step
-                            const uint32_t first = (kb | k) ? 1u : 0u;              // first MMA of this chunk
-                            if (DRAIN) {
-                                const uint32_t first_u = ((kb0 + kb) | k) ? 1u : 0u; // first MMA of this unit
-                                if (passes == 3) {
-                                    tc::umma_tf32(d_small, a_lo + koff, b_hi + koff, idesc, first_u);
-                                    tc::umma_tf32(d_small, a_raw + koff, b_lo + koff, idesc, 1u);
-                                } else {
-                                    tc::umma_tf32(d_small, a_raw + koff, b_lo + koff, idesc, first_u);
-                                }
-                                tc::umma_tf32(d_tmem, a_raw + koff, b_hi + koff, idesc, first);
-                            } else if (bf16) {
-                                // bf16 storage: Phi is exact in bf16, the plan operand is a bf16 hi/lo pair; 16 elements per k-step
-                                tc::umma_f16(d_tmem, a_raw + koff, b_lo + koff, idesc, first);
-                                tc::umma_f16(d_tmem, a_raw + koff, b_hi + koff, idesc, 1u);
-                            } else {
-                                if (passes == 3) {
-                                    tc::umma_tf32(d_tmem, a_lo + koff, b_hi + koff, idesc, first);
-                                    tc::umma_tf32(d_tmem, a_raw + koff, b_lo + koff, idesc, 1u);
-                                } else {
-                                    tc::umma_tf32(d_tmem, a_raw + koff, b_lo + koff, idesc, first);
-                                }
-                                tc::umma_tf32(d_tmem, a_raw + koff, b_hi + koff, idesc, 1u);
-                            }
-                        }
-                        tc::umma_commit(&ctrl->empty[s]);
-                        if (++s == n_stages) { s = 0; ph ^= 1; }
-                    }
-                    tc::umma_commit(&ctrl->tmem_full[a]);
-                    if (++a == 2) { a = 0; aph ^= 1; }
-                }
-                if (DRAIN) {
-                    tc::umma_commit(&ctrl->small_full[b]);
-                    if (++b == 2) { b = 0; bph ^= 1; }
-                }
-            }
-        }
-    } else if (warp < 6) {
-        // ------------------------------------------------------------ converter: hi/lo split of the big operand
-        if (passes == 3) {
-            const int tid = threadIdx.x - 64;          // 0..127
-            int s = 0; uint32_t ph = 0;
-            for (int u = unit_begin; u < unit_end; ++u) {
-                const TcUnit un = L.units[u];
-                const int nvec = ((un.rows + kBoxRows - 1) / kBoxRows) * (kBoxBytes / 16);
+                tc::mbar_wait(&ctrl->tmem_empty[a], aph ^ 1);
+                tc::tcgen05_fence_after();
+                const uint32_t d_tmem = tmem_base + a * kAccCols;
                 for (int kb = 0; kb < un.kb_count; ++kb) {
                     tc::mbar_wait(&ctrl->full[s], ph);
-                    float4* raw = reinterpret_cast<float4*>(stage_a_raw(s));
-                    float4* lo = reinterpret_cast<float4*>(stage_a_lo(s));
-#pragma unroll 4
-                    for (int i = tid; i < nvec; i += 128) {
-                        float4 v = raw[i];
-                        float4 hi, l;
-                        hi.x = __uint_as_float(__float_as_uint(v.x) & 0xFFFFE000u); l.x = v.x - hi.x;
-                        hi.y = __uint_as_float(__float_as_uint(v.y) & 0xFFFFE000u); l.y = v.y - hi.y;
-                        hi.z = __uint_as_float(__float_as_uint(v.z) & 0xFFFFE000u); l.z = v.z - hi.z;
-                        hi.w = __uint_as_float(__float_as_uint(v.w) & 0xFFFFE000u); l.w = v.w - hi.w;
-                        raw[i] = hi;
-                        lo[i] = l;
+                    tc::tcgen05_fence_after();
+                    const uint64_t a_desc = tc::umma_desc_k_sw128(tc::smem_u32(stage_a(s)));
+                    const uint64_t b_hi = tc::umma_desc_k_sw128(tc::smem_u32(stage_b_hi(s)));
+                    const uint64_t b_lo = tc::umma_desc_k_sw128(tc::smem_u32(stage_b_lo(s)));
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const uint64_t koff = (uint64_t)(2 * k);                // 32 bytes per k-step (8 tf32 / 16 bf16 elements)
+                        const uint32_t first = (kb | k) ? 1u : 0u;              // first MMA of this unit overwrites
+                        if (bf16) {
+                            tc::umma_f16(d_tmem, a_desc + koff, b_lo + koff, idesc, first);
+                            tc::umma_f16(d_tmem, a_desc + koff, b_hi + koff, idesc, 1u);
+                        } else {
+                            tc::umma_tf32(d_tmem, a_desc + koff, b_lo + koff, idesc, first);
+                            tc::umma_tf32(d_tmem, a_desc + koff, b_hi + koff, idesc, 1u);
+                        }
                     }
-                    tc::fence_proxy_async_smem();
-                    tc::mbar_arrive(&ctrl->conv[s]);
+                    tc::umma_commit(&ctrl->empty[s]);
                     if (++s == n_stages) { s = 0; ph ^= 1; }
                 }
+                tc::umma_commit(&ctrl->tmem_full[a]);
+                if (++a == 2) { a = 0; aph ^= 1; }
             }
         }
-    } else {
+    } else if (warp >= 6) {
         // ------------------------------------------------------------ epilogue (one TMEM lane = one row per thread)
         const int ew = warp & 3;                       // TMEM lane group this warp may read
         const EpiParams& ep = L.ep;
         const int n16 = n_mma / 16;
-        const int half = DRAIN ? ((warp - 6) >> 2) : 0;
-        const int cbeg = DRAIN ? (half == 0 ? 0 : (n16 + 1) / 2) : 0;          // first 16-column group of this warp
-        const int cend = DRAIN ? (half == 0 ? (n16 + 1) / 2 : n16) : n16;
         EpiCtx cx;
         cx.lane = lane;
+        cx.n_act = n_act;
         cx.wacc = acc + (warp - 6) * n_mma * 8;
         cx.resid = (L.epi == EPI_K3_STATE) && (ep.resid_partial != nullptr);
         int a = 0; uint32_t aph = 0;
-        int b2 = 0; uint32_t bph2 = 0;
         for (int u = unit_begin; u < unit_end; ++u) {
             const TcUnit un = L.units[u];
             cx.lrow = ew * 32 + lane;
@@ -326,76 +252,34 @@ __global__ void __launch_bounds__(DRAIN ? 448 : 320, 1) admm_contract_kernel(con
             cx.a_k = ep.a_cls[cx.cls]; cx.sense = ep.sense[cx.cls]; cx.thr = ep.thr[cx.cls];
             cx.mword = cx.row >> 5;
             const uint32_t lane_addr = tmem_base + ((uint32_t)(ew * 32) << 16);
-            if (DRAIN) {
-                float master[64];
+            tc::mbar_wait(&ctrl->tmem_full[a], aph);
+            tc::tcgen05_fence_after();
+            for (int c = 0; c < n16; ++c) {
+                uint32_t r[16];
+                tc::tmem_ld16(lane_addr + a * kAccCols + c * 16, r);
+                tc::tmem_ld_wait(r);
+                float q[16];
 #pragma unroll
-                for (int i = 0; i < 64; ++i) master[i] = 0.0f;
-                for (int kb0 = 0; kb0 < un.kb_count; kb0 += chunk_kb) {
-                    tc::mbar_wait(&ctrl->tmem_full[a], aph);
-                    tc::tcgen05_fence_after();
-#pragma unroll
-                    for (int cc = 0; cc < 4; ++cc) {
-                        if (cbeg + cc < cend) {
-                            uint32_t r[16];
-                            tc::tmem_ld16(lane_addr + a * kDrainCols + (cbeg + cc) * 16, r);
-                            tc::tmem_ld_wait(r);
-#pragma unroll
-                            for (int jj = 0; jj < 16; ++jj) master[cc * 16 + jj] += __uint_as_float(r[jj]);
-                        }
-                    }
-                    tc::tcgen05_fence_before();
-                    tc::mbar_arrive(&ctrl->tmem_empty[a]);
-                    if (++a == 2) { a = 0; aph ^= 1; }
-                }
-                // the correction-term accumulator of this unit
-                tc::mbar_wait(&ctrl->small_full[b2], bph2);
-                tc::tcgen05_fence_after();
-#pragma unroll
-                for (int cc = 0; cc < 4; ++cc) {
-                    if (cbeg + cc < cend) {
-                        uint32_t r[16];
-                        tc::tmem_ld16(lane_addr + 2 * kDrainCols + b2 * kDrainCols + (cbeg + cc) * 16, r);
-                        tc::tmem_ld_wait(r);
-#pragma unroll
-                        for (int jj = 0; jj < 16; ++jj) master[cc * 16 + jj] += __uint_as_float(r[jj]);
-                    }
-                }
-                tc::tcgen05_fence_before();
-                tc::mbar_arrive(&ctrl->small_empty[b2]);
-                if (++b2 == 2) { b2 = 0; bph2 ^= 1; }
-#pragma unroll
-                for (int cc = 0; cc < 4; ++cc)
-                    if (cbeg + cc < cend) epi_cols16(L, cx, (cbeg + cc) * 16, *reinterpret_cast<const float(*)[16]>(&master[cc * 16]));
-            } else {
-                tc::mbar_wait(&ctrl->tmem_full[a], aph);
-                tc::tcgen05_fence_after();
-                for (int c = cbeg; c < cend; ++c) {
-                    uint32_t r[16];
-                    tc::tmem_ld16(lane_addr + a * kAccCols + c * 16, r);
-                    tc::tmem_ld_wait(r);
-                    float q[16];
-#pragma unroll
-                    for (int jj = 0; jj < 16; ++jj) q[jj] = __uint_as_float(r[jj]);
-                    epi_cols16(L, cx, c * 16, q);
-                }
-                tc::tcgen05_fence_before();
-                tc::mbar_arrive(&ctrl->tmem_empty[a]);
-                if (++a == 2) { a = 0; aph ^= 1; }
+                for (int jj = 0; jj < 16; ++jj) q[jj] = __uint_as_float(r[jj]);
+                epi_cols16(L, cx, c * 16, q);
             }
+            tc::tcgen05_fence_before();
+            tc::mbar_arrive(&ctrl->tmem_empty[a]);
+            if (++a == 2) { a = 0; aph ^= 1; }
         }
     }
 
     __syncthreads();
     // per-CTA partial sums -> global (fixed order over the epilogue warps), deterministic
     if (L.epi == EPI_K3_STATE && L.ep.resid_partial != nullptr) {
-        for (int i = threadIdx.x; i < L.ep.n_slots_active * kNumResid; i += kThreads) {
+        for (int i = threadIdx.x; i < n_act * kNumResid; i += kThreads) {
             const int p = i / kNumResid, t = i % kNumResid;
             float v = 0.f;
             for (int w = 0; w < kEpiWarps; ++w) v += acc[(w * n_mma + p) * 8 + t];
             L.ep.resid_partial[((int64_t)blockIdx.x * kMaxBpad + L.ep.slot0 + p) * kNumResid + t] = v;
         }
     } else if (L.epi == EPI_OBJECTIVE) {
-        for (int i = threadIdx.x; i < L.ep.n_slots_active * kMaxClasses; i += kThreads) {
+        for (int i = threadIdx.x; i < n_act * kMaxClasses; i += kThreads) {
             const int p = i / kMaxClasses, k = i % kMaxClasses;
             double v = 0.0;
             for (int w = 0; w < kEpiWarps; ++w) v += (double)acc[(w * n_mma + p) * 8 + k];
@@ -633,6 +517,8 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
     const int unit_begin = L.cta_unit_begin[blockIdx.x];
     const int unit_end = L.cta_unit_begin[blockIdx.x + 1];
     const int chunk_kb = L.chunk_kb;
+    const int n_act = eff_nact(L.ep);
+    if (n_act <= 0) return;                               // the whole pass froze since the host sized this launch
 
     if (threadIdx.x == 0) {
         // sa_empty: released by the 4 converter warps (3xTF32: the raw tile is in registers) or by the MMA commit (direct mode)
@@ -911,7 +797,6 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
         // ------------------------------------------------------------ epilogue warps: qs -> global, concurrent with the next unit
         const int wq = (warp - kEpiWarp0) & 3;           // row quarter
         const int ph_half = (warp - kEpiWarp0) >> 2;     // which half of the plans
-        const int n_act = L.ep.n_slots_active;
         const int p_mid = (n_act + 1) / 2;
         const int p_begin = ph_half == 0 ? 0 : p_mid;
         const int p_end = ph_half == 0 ? p_mid : n_act;
@@ -930,14 +815,14 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
 
     __syncthreads();
     if (L.epi == EPI_K3_STATE && L.ep.resid_partial != nullptr) {
-        for (int i = threadIdx.x; i < L.ep.n_slots_active * kNumResid; i += kF32Threads) {
+        for (int i = threadIdx.x; i < n_act * kNumResid; i += kF32Threads) {
             const int p = i / kNumResid, t = i % kNumResid;
             float v = 0.f;
             for (int w = 0; w < 8; ++w) v += acc[(w * n_mma + p) * 8 + t];
             L.ep.resid_partial[((int64_t)blockIdx.x * kMaxBpad + L.ep.slot0 + p) * kNumResid + t] = v;
         }
     } else if (L.epi == EPI_OBJECTIVE) {
-        for (int i = threadIdx.x; i < L.ep.n_slots_active * kMaxClasses; i += kF32Threads) {
+        for (int i = threadIdx.x; i < n_act * kMaxClasses; i += kF32Threads) {
             const int p = i / kMaxClasses, k = i % kMaxClasses;
             double v = 0.0;
             for (int w = 0; w < 8; ++w) v += (double)acc[(w * n_mma + p) * 8 + k];
@@ -969,7 +854,7 @@ admm_status tc_init(admm_handle* h) {
         g_encode = reinterpret_cast<EncodeTiledFn>(fn);
     }
     cudaError_t e = cudaFuncSetAttribute(admm_contract_f32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(admm_contract_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(admm_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
     if (e != cudaSuccess) {
         h->err = std::string("cudaFuncSetAttribute(max dynamic smem): ") + cudaGetErrorString(e);
         return ADMM_ECUDA;
@@ -1004,9 +889,7 @@ admm_status tc_launch(admm_handle* h, const TcLaunch& L) {
         h->err = "tc_launch: n_mma must be a multiple of 16 in [16, 256]";
         return ADMM_EINVAL;
     }
-    const int sbytes = stage_bytes(L.mma_passes, n_mma);
-    int n_stages = (kSmemLimit - 1024 - (int)sizeof(Ctrl) - acc_bytes(n_mma)) / sbytes;
-    if (n_stages < 2) {
+    if ((kSmemLimit - 1024 - (int)sizeof(Ctrl) - acc_bytes(n_mma)) / stage_bytes(n_mma) < 2) {
         h->err = "tc_launch: fewer than 2 pipeline stages fit in shared memory";
         return ADMM_EINVAL;
     }
@@ -1023,7 +906,7 @@ admm_status tc_launch(admm_handle* h, const TcLaunch& L) {
         if (L.mma_passes == 3 && L2.n_sb == 3) L2.n_sb = 2;
         admm_contract_f32_kernel<<<L.grid, kF32Threads, kSmemLimit, h->stream>>>(L2);
     } else {
-        admm_contract_kernel<false><<<L.grid, 320, kSmemLimit, h->stream>>>(L);
+        admm_contract_kernel<<<L.grid, 320, kSmemLimit, h->stream>>>(L);
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) {

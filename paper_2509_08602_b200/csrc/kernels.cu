@@ -1,6 +1,7 @@
 // Everything on the hot path that is not a tcgen05 contraction: the S^-1 apply with fused epilogue-2
 // (K2a/K2b), the stopping rule, state start-up / read-out, setup helpers, and the plain-FFMA
 // cross-check versions of K1/K3 (ADMM_PATH_SIMT).
+#include <algorithm>
 #include <cstdio>
 #include "admm_internal.h"
 #include "epilogue.cuh"
@@ -171,8 +172,9 @@ __global__ void emit_g_kernel(const EpiParams ep, int Bact) {
 }
 
 __global__ void state_out_kernel(const EpiParams ep, int slot, const double* __restrict__ s2, const double* __restrict__ R,
-                                 double beta, float* z1, float* y1, double* z2, double* y2) {
+                                 const double* __restrict__ beta_tab, float* z1, float* y1, double* z2, double* y2) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const double beta = beta_tab[slot];
     if (i < ep.N && (z1 || y1)) {
         int cls = ep.point_class[i];
         float ub = mask_ub(ep, cls, slot, i);
@@ -206,9 +208,11 @@ __global__ void make_t_kernel(const double* __restrict__ s2, const double* __res
 // rhs[p][j] = R_j * sum_slots partial[slot][p][j - 128 mt]  -  (2 z2 - s2)[p][j]     (fp64)
 __global__ void k2a_kernel(const float* __restrict__ partial, const int32_t* __restrict__ mtile_slot_begin, int n_mma,
                            const double* __restrict__ s2, const double* __restrict__ R, const double* __restrict__ beta,
-                           int64_t n, int64_t ldn, int slot0, int nact, double* __restrict__ rhs) {
+                           int64_t n, int64_t ldn, int slot0, int nact, const int32_t* __restrict__ bact_dev,
+                           double* __restrict__ rhs) {
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int p = blockIdx.y;                       // index inside this contraction pass
+    if (bact_dev) nact = min(nact, *bact_dev - slot0);
     if (j >= n || p >= nact) return;
     int mt = (int)(j / kTileM), jl = (int)(j % kTileM);
     double w = 0.0;
@@ -252,9 +256,11 @@ template <int WJ>
 __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sinv, int64_t lds,
                                                   const double* __restrict__ rhs, double* __restrict__ s2,
                                                   const double* __restrict__ R, const double* __restrict__ beta,
-                                                  int64_t n, int64_t ldn, int Bact,
+                                                  int64_t n, int64_t ldn, int Bact, const int32_t* __restrict__ bact_dev,
                                                   void* __restrict__ v_hi, void* __restrict__ v_lo, int bf16,
                                                   double* __restrict__ resid_partial) {
+    if (bact_dev) Bact = min(Bact, *bact_dev);             // the host's bound lags the device by up to one check interval
+    if ((int)blockIdx.y * K2_TP >= Bact) return;
     // 8 warps = WJ row groups x 2 plan halves x KS k-slices (a lone warp per scheduler cannot hide the DMMA issue
     // latency: measured 14 % pipe utilisation with 2 warps per block); the k-slices are summed through shared memory.
     constexpr int TJ = 16 * WJ, NT = 256, ROWS = TJ + K2_TP, KS = 4 / WJ, K2_STAGES = k2_stages(WJ);
@@ -406,14 +412,17 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
     }
 }
 
-// ------------------------------------------------------------------------------------------ stopping rule (R7)
+// ------------------------------------------------------------------------------------------ stopping rule (R7) + compaction (H5)
 // One warp per slot: the per-CTA partials of both blocks are summed in a fixed order (lane-strided, then a butterfly),
-// so the decision is deterministic; then the Boyd test.
+// so the decision is deterministic; then the Boyd test.  Also records, per PLAN, the iteration count and the residual norms of
+// every live plan at this check (a plan that freezes now keeps these values).
 __global__ void convergence_kernel(const float* __restrict__ r1, int grid1, const double* __restrict__ r2, int grid2,
-                                   int Bact, double dim_sqrt, float tol, float eps_abs,
-                                   int32_t* __restrict__ flags, float* __restrict__ res_slot) {
+                                   const int32_t* __restrict__ bact_dev, int Bact, double dim_sqrt, float tol, float eps_abs, int it,
+                                   const int32_t* __restrict__ slot_plan, int32_t* __restrict__ flags,
+                                   int32_t* __restrict__ iters_plan, float* __restrict__ res_plan) {
     const int p = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
+    if (bact_dev) Bact = min(Bact, *bact_dev);
     if (p >= Bact) return;
     double a[kNumResid] = {0, 0, 0, 0, 0};
     for (int g = lane; g < grid1; g += 32)
@@ -425,9 +434,122 @@ __global__ void convergence_kernel(const float* __restrict__ r1, int grid1, cons
     const double rp = sqrt(a[0]), rd = sqrt(a[1]), nx = sqrt(a[2]), nz = sqrt(a[3]), ny = sqrt(a[4]);
     const bool ok = (rp <= (double)eps_abs * dim_sqrt + (double)tol * fmax(nx, nz)) &&
                     (rd <= (double)eps_abs * dim_sqrt + (double)tol * ny);
-    flags[p] = ok ? 1 : 0;
-    res_slot[2 * p] = (float)rp;
-    res_slot[2 * p + 1] = (float)rd;
+    flags[p] = (ok && tol > 0.f) ? 1 : 0;
+    const int plan = slot_plan[p];
+    iters_plan[plan] = it;
+    res_plan[2 * plan] = (float)rp;
+    res_plan[2 * plan + 1] = (float)rd;
+}
+
+// Compaction decided on the device (one thread: at most 496 slots, a few table entries each).  With L live plans left after
+// this check, the live range becomes [0, L): every flagged slot below L (a hole) trades places with an unflagged slot at or above L
+// (a mover), so a frozen plan keeps its state (the iterate that passed the test) behind the live range.  Holes and movers are all
+// different slots, so the row moves (move_rows_kernel, from the list written here) are independent of one another.
+__global__ void compact_kernel(int32_t* __restrict__ bact, const int32_t* __restrict__ flags, int32_t* __restrict__ slot_plan,
+                               float* __restrict__ utab, float* __restrict__ crtab, double* __restrict__ beta,
+                               double* __restrict__ rho, double* __restrict__ wnorm, int32_t* __restrict__ moves,
+                               int32_t* __restrict__ nmoves) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const int B = *bact;
+    int live = 0, nm = 0;
+    for (int s = 0; s < B; ++s) live += flags[s] ? 0 : 1;
+    int mover = B - 1;
+    for (int hole = 0; hole < live; ++hole) {
+        if (!flags[hole]) continue;
+        while (flags[mover]) --mover;                       // an unflagged slot >= live exists for every hole
+        const int s = hole, last = mover;
+        for (int k = 0; k < kMaxClasses; ++k) {
+            float tu = utab[k * kMaxBpad + s]; utab[k * kMaxBpad + s] = utab[k * kMaxBpad + last]; utab[k * kMaxBpad + last] = tu;
+            float tcr = crtab[k * kMaxBpad + s]; crtab[k * kMaxBpad + s] = crtab[k * kMaxBpad + last]; crtab[k * kMaxBpad + last] = tcr;
+            double tw = wnorm[s * kMaxClasses + k]; wnorm[s * kMaxClasses + k] = wnorm[last * kMaxClasses + k]; wnorm[last * kMaxClasses + k] = tw;
+        }
+        double tb = beta[s]; beta[s] = beta[last]; beta[last] = tb;
+        double tr = rho[s]; rho[s] = rho[last]; rho[last] = tr;
+        int tp = slot_plan[s]; slot_plan[s] = slot_plan[last]; slot_plan[last] = tp;
+        moves[2 * nm] = s; moves[2 * nm + 1] = last; ++nm;
+        --mover;
+    }
+    *bact = live;
+    *nmoves = nm;
+}
+
+// move m: frozen slot a (a hole) <-> live slot b (its mover).  s1 and s2 are swapped (the frozen state is an output); the K1 operand G only moves
+// b -> a (a frozen plan needs no operand).  Rows are walked as 16-byte words; grid = (chunks, upper bound on the moves).
+__global__ void move_rows_kernel(const int32_t* __restrict__ moves, const int32_t* __restrict__ nmoves, float4* __restrict__ s1,
+                                 float4* __restrict__ ghi, float4* __restrict__ glo, int64_t ldN4, double2* __restrict__ s2, int64_t ldn2) {
+    const int m = blockIdx.y;
+    if (m >= *nmoves) return;
+    const int a = moves[2 * m], b = moves[2 * m + 1];
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x, t0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    float4* sa = s1 + (int64_t)a * ldN4; float4* sb = s1 + (int64_t)b * ldN4;
+    float4* ha = ghi + (int64_t)a * ldN4; const float4* hb = ghi + (int64_t)b * ldN4;
+    float4* la = glo + (int64_t)a * ldN4; const float4* lb = glo + (int64_t)b * ldN4;
+    for (int64_t i = t0; i < ldN4; i += stride) {
+        const float4 x = sa[i], y = sb[i];
+        sa[i] = y; sb[i] = x;
+        ha[i] = hb[i]; la[i] = lb[i];
+    }
+    double2* qa = s2 + (int64_t)a * ldn2; double2* qb = s2 + (int64_t)b * ldn2;
+    for (int64_t i = t0; i < ldn2; i += stride) {
+        const double2 x = qa[i], y = qb[i];
+        qa[i] = y; qb[i] = x;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ presolve: the box optimum
+// x_box = argmin c^T x over the box alone (x = u where c < 0, 0 where c > 0; Eq. 1).  If A x_box <= b it is optimal
+// for the LP, t* = 0, and the ADMM fixed point is known in closed form: z1 = x_box, y1 = -c/rho, z2 = A x_box, y2 = 0 (Eq. 6-7 with
+// v = y2 = 0).  presolve_state_kernel writes s1 = z1 + y1 of that candidate for every plan (emit_g then yields G = a o z1, and the K1
+// contraction A^ z1); presolve_test_kernel accepts a plan iff A^ z1 <= b^ (1 - margin) in every row and then stores s2 = z2.
+__global__ void presolve_state_kernel(const EpiParams ep, int B) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int p = blockIdx.y;
+    if (i >= ep.N || p >= B) return;
+    const int cls = ep.point_class[i];
+    const float cr = ep.crtab[cls * kMaxBpad + p];
+    const float ub = mask_ub(ep, cls, p, i);
+    ep.s1[(int64_t)p * ep.ldN + i] = (cr < 0.f ? ub : 0.f) - cr;
+}
+// one block per plan
+__global__ void presolve_test_kernel(const float* __restrict__ partial, const int32_t* __restrict__ mtile_slot_begin, int n_mma,
+                                     const double* __restrict__ R, const double* __restrict__ beta, int64_t n, int64_t ldn,
+                                     int slot0, int nact, double margin, double* __restrict__ s2, int32_t* __restrict__ flags) {
+    const int p = blockIdx.x;
+    if (p >= nact) return;
+    const int gs = slot0 + p;
+    __shared__ int bad;
+    if (threadIdx.x == 0) bad = 0;
+    __syncthreads();
+    const double bp = beta[gs];
+    int mybad = 0;
+    for (int64_t j = threadIdx.x; j < n; j += blockDim.x) {
+        const int mt = (int)(j / kTileM), jl = (int)(j % kTileM);
+        double w = 0.0;
+        for (int s = mtile_slot_begin[mt]; s < mtile_slot_begin[mt + 1]; ++s)
+            w += (double)partial[((int64_t)s * n_mma + p) * kTileM + jl];
+        w *= R[j];
+        if (!(w <= R[j] * bp * (1.0 - margin))) mybad = 1;
+        s2[(int64_t)gs * ldn + j] = w;                     // z2 of the candidate; overwritten with 0 below if it is rejected
+    }
+    if (mybad) bad = 1;
+    __syncthreads();
+    const int rejected = bad;
+    if (rejected)
+        for (int64_t j = threadIdx.x; j < n; j += blockDim.x) s2[(int64_t)gs * ldn + j] = 0.0;
+    if (threadIdx.x == 0) flags[gs] = rejected ? 0 : 1;
+}
+// zero start (R6) for the plans the presolve did not accept; their K1 operand is re-emitted by emit_g afterwards
+__global__ void presolve_reset_kernel(const int32_t* __restrict__ flags, float* __restrict__ s1, int64_t N, int64_t ldN, int B) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int p = blockIdx.y;
+    if (i >= N || p >= B || flags[p]) return;
+    s1[(int64_t)p * ldN + i] = 0.f;
+}
+__global__ void set_iters_kernel(const int32_t* __restrict__ flags, int B, int32_t* __restrict__ iters_plan, float* __restrict__ res_plan) {
+    int p = blockIdx.x * blockDim.x + threadIdx.x;        // slot == plan before any compaction
+    if (p >= B) return;
+    iters_plan[p] = 0; res_plan[2 * p] = 0.f; res_plan[2 * p + 1] = 0.f;
+    (void)flags;
 }
 
 // ------------------------------------------------------------------------------------------ SIMT cross-check contractions
@@ -631,7 +753,7 @@ void launch_emit_g(const EpiParams& ep, int Bact, cudaStream_t s) {
 void launch_k2a(admm_handle* h, int slot0, int nact, int n_mma, cudaStream_t s) {
     dim3 grid((unsigned)cdiv(h->n, 128), nact);
     k2a_kernel<<<grid, 128, 0, s>>>(h->d_partial, h->d_mtile_slot_begin, n_mma, h->d_s2, h->d_R, h->d_beta, h->n, h->ldn,
-                                    slot0, nact, h->d_rhs);
+                                    slot0, nact, h->d_bact, h->d_rhs);
     h->launch_count++;
 }
 // rows of the block tile: the largest of 64 / 32 / 16 that still gives every SM a block
@@ -646,10 +768,10 @@ int k2b_grid(const admm_handle* h, int) { return (int)cdiv(h->n, 16 * k2_wj(h));
 template <int WJ>
 static void launch_k2b_t(admm_handle* h, int Bact, bool resid, cudaStream_t s) {
     const size_t smem = (size_t)k2_stages(WJ) * (16 * WJ + K2_TP) * K2_LD * sizeof(double);
-    static bool attr_done = false;
-    if (!attr_done) { cudaFuncSetAttribute(k2b_kernel<WJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_done = true; }
+    // the attribute is per device: set it once per handle (a process-wide flag would leave a second device without the opt-in)
+    if (!h->k2_attr_set) { cudaFuncSetAttribute(k2b_kernel<WJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); h->k2_attr_set = true; }
     dim3 grid((unsigned)cdiv(h->n, 16 * WJ), (unsigned)cdiv(Bact, K2_TP));
-    k2b_kernel<WJ><<<grid, 256, smem, s>>>(h->d_Sinv, h->lds, h->d_rhs, h->d_s2, h->d_R, h->d_beta, h->n, h->ldn, Bact,
+    k2b_kernel<WJ><<<grid, 256, smem, s>>>(h->d_Sinv, h->lds, h->d_rhs, h->d_s2, h->d_R, h->d_beta, h->n, h->ldn, Bact, h->d_bact,
                                                h->d_vhi, h->d_vlo, h->opt.storage == ADMM_STORAGE_BF16 ? 1 : 0,
                                                resid ? h->d_resid2 : nullptr);
 }
@@ -686,11 +808,37 @@ void launch_simt_k3(admm_handle* h, const EpiParams& ep, int epi, const float* v
     simt_epilogue_kernel<<<(unsigned)cdiv(h->N, 128), 128, 0, s>>>(ep, epi, qbuf);
     h->launch_count += 2;
 }
-void launch_convergence(admm_handle* h, int Bact, int grid1, int grid2, float tol, float eps_abs, cudaStream_t s) {
-    convergence_kernel<<<(unsigned)cdiv(Bact, 4), 128, 0, s>>>(h->d_resid1, grid1, h->d_resid2, grid2, Bact,
-                                                              sqrt((double)(h->N + h->n)), tol, eps_abs, h->d_conv_flags,
-                                                              h->d_res_slot);
+void launch_convergence(admm_handle* h, int Bact, int grid1, int grid2, float tol, float eps_abs, int it, cudaStream_t s) {
+    convergence_kernel<<<(unsigned)cdiv(Bact, 4), 128, 0, s>>>(h->d_resid1, grid1, h->d_resid2, grid2, h->d_bact, Bact,
+                                                              sqrt((double)(h->N + h->n)), tol, eps_abs, it, h->d_slot_plan,
+                                                              h->d_conv_flags, h->d_iters_plan, h->d_res_plan);
     h->launch_count++;
+}
+// H5 on the device: shrink the live range, fix the per-slot tables, move the rows.  `Bact` is the host's upper bound on the live count.
+void launch_compaction(admm_handle* h, int Bact, cudaStream_t s) {
+    compact_kernel<<<1, 32, 0, s>>>(h->d_bact, h->d_conv_flags, h->d_slot_plan, h->d_utab, h->d_crtab, h->d_beta, h->d_rho,
+                                    h->d_wnorm, h->d_moves, h->d_nmoves);
+    const int64_t ldN4 = h->ldN / 4, ldn2 = h->ldn / 2;
+    const unsigned gx = (unsigned)std::max<int64_t>(1, std::min<int64_t>(64, cdiv(ldN4, 256)));
+    move_rows_kernel<<<dim3(gx, (unsigned)std::max(1, Bact / 2)), 256, 0, s>>>(
+        h->d_moves, h->d_nmoves, reinterpret_cast<float4*>(h->d_s1), reinterpret_cast<float4*>(h->d_ghi),
+        reinterpret_cast<float4*>(h->d_glo), ldN4, reinterpret_cast<double2*>(h->d_s2), ldn2);
+    h->launch_count += 2;
+}
+void launch_presolve_state(const EpiParams& ep, int B, cudaStream_t s) {
+    dim3 grid((unsigned)cdiv(ep.N, 256), B);
+    presolve_state_kernel<<<grid, 256, 0, s>>>(ep, B);
+}
+void launch_presolve_test(admm_handle* h, int slot0, int nact, int n_mma, double margin, cudaStream_t s) {
+    presolve_test_kernel<<<nact, 256, 0, s>>>(h->d_partial, h->d_mtile_slot_begin, n_mma, h->d_R, h->d_beta, h->n, h->ldn, slot0, nact,
+                                               margin, h->d_s2, h->d_conv_flags);
+}
+void launch_presolve_reset(admm_handle* h, int B, cudaStream_t s) {
+    dim3 grid((unsigned)cdiv(h->N, 256), B);
+    presolve_reset_kernel<<<grid, 256, 0, s>>>(h->d_conv_flags, h->d_s1, h->N, h->ldN, B);
+}
+void launch_init_plan_records(admm_handle* h, int B, cudaStream_t s) {
+    set_iters_kernel<<<(unsigned)cdiv(B, 128), 128, 0, s>>>(h->d_conv_flags, B, h->d_iters_plan, h->d_res_plan);
 }
 void launch_make_t(admm_handle* h, int Bact, void* t_hi, void* t_lo, float* t_f32, cudaStream_t s) {
     dim3 grid((unsigned)cdiv(h->n, 128), Bact);
@@ -714,8 +862,8 @@ void launch_gather_rows(const float* src, int64_t ld, const int32_t* plan_slot, 
     dim3 grid((unsigned)cdiv(n, 256), B);
     gather_rows_kernel<<<grid, 256, 0, s>>>(src, ld, plan_slot, B, n, dst);
 }
-void launch_state_out(admm_handle* h, const EpiParams& ep, int slot, double beta, float* z1, float* y1, double* z2,
+void launch_state_out(admm_handle* h, const EpiParams& ep, int slot, float* z1, float* y1, double* z2,
                       double* y2, cudaStream_t s) {
     int64_t m = h->N > h->n ? h->N : h->n;
-    state_out_kernel<<<(unsigned)cdiv(m, 256), 256, 0, s>>>(ep, slot, h->d_s2, h->d_R, beta, z1, y1, z2, y2);
+    state_out_kernel<<<(unsigned)cdiv(m, 256), 256, 0, s>>>(ep, slot, h->d_s2, h->d_R, h->d_beta, z1, y1, z2, y2);
 }

@@ -302,19 +302,53 @@ def test_converged_objectives_match_simplex_config0(b):
     assert conv.sum() >= 7 and np.all(out["iters"][conv] % 10 == 0)
     assert np.all(err[conv] < 1e-3), err
     # iteration counts: the decision is taken on fp32 data, the oracle's in fp64 -> same count up to one test interval
-    ref = _oracle(w, rho, 3000, tol=1e-4)
+    ref = _oracle(w, rho, 3000, tol=1e-4, presolve=True)
     both = conv & ref["converged"]
     assert both.sum() >= 7
     assert np.all(np.abs(out["iters"][both] - ref["iters"][both]) <= 20), (out["iters"], ref["iters"])
+    # the presolve (deviation D1) takes the same decision on both sides (config 0: max_j mean_T Phi_j > 1, no plan is settled by it)
+    assert np.array_equal(out["iters"] == 0, ref["presolved"])
+
+
+def test_presolve_matches_oracle(b):
+    """Deviation D1: plans whose box optimum is feasible are settled before iterating, with the ADMM fixed point as their state
+    (oracle/admm.py presolve_box_optimum); the other plans are not touched by the option (bit-identical to presolve off)."""
+    from oracle import admm
+    from workloads import default_rho, make_workload, pack_mask
+    w = make_workload(2, n_target=900, n_lowdose=1800, n_iso=9, grid=5)     # 9 targets, row masks, beta in {0, .25, .5, .75, 1}
+    rho = default_rho(w.beta)
+    ref = _oracle(w, rho, 200, tol=1e-3, presolve=True)
+    assert 0 < ref["presolved"].sum() < w.B
+    h = b.admm_setup(w.phi, w.point_class, w.classes)
+    on = b.admm_solve_batch(h, w.weights, rho, w.row_mask, tol=1e-3, max_iter=200)
+    st_on = _gpu_states(b, h, w.B)
+    assert np.array_equal(on["iters"] == 0, ref["presolved"])
+    for p in np.nonzero(ref["presolved"])[0]:
+        z1, y1, z2, y2 = st_on[p]
+        assert np.all(on["t"][p] == 0) and np.all(y2 == 0)
+        assert np.allclose(z1, ref["z1"][:, p], rtol=1e-6, atol=1e-9) and np.allclose(y1, ref["y1"][:, p], rtol=1e-6)
+        assert np.allclose(z2, ref["z2"][:, p], rtol=1e-5, atol=1e-9 * np.abs(ref["z2"][:, p]).max())
+        assert abs(on["obj"][p] - ref["obj"][p]) < 1e-6
+    h.close()
+    h = b.admm_setup(w.phi, w.point_class, w.classes, presolve=False)
+    off = b.admm_solve_batch(h, w.weights, rho, w.row_mask, tol=1e-3, max_iter=200)
+    st_off = _gpu_states(b, h, w.B)
+    h.close()
+    assert np.all(off["iters"] > 0)
+    for p in np.nonzero(~ref["presolved"])[0]:
+        assert on["iters"][p] == off["iters"][p] and np.array_equal(on["t"][p], off["t"][p])
+        for a, c in zip(st_on[p], st_off[p]):
+            assert np.array_equal(a, c)
 
 
 def test_compaction_preserves_each_plan(b):
-    """A plan frozen and swapped out at iteration k must equal the same plan run alone for k iterations,
-    and plans that keep iterating must not be disturbed by the swaps (plans are independent columns, :96)."""
+    """A plan frozen and moved out of the live range at iteration k (on the device: compact_kernel + move_rows_kernel) must equal
+    the same plan run alone for k iterations, and plans that keep iterating must not be disturbed by the moves (plans are
+    independent columns, :96)."""
     from workloads import default_rho, make_workload
     w = make_workload(0, n_target=500, n_lowdose=900, n_iso=5)
     rho = default_rho(w.beta)
-    h = b.admm_setup(w.phi, w.point_class, w.classes)
+    h = b.admm_setup(w.phi, w.point_class, w.classes, presolve=False)
     out = b.admm_solve_batch(h, w.weights, rho, tol=1e-3, max_iter=400)
     iters = out["iters"].copy()
     states = _gpu_states(b, h, w.B)

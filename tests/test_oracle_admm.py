@@ -187,3 +187,69 @@ def test_stopping_rule_freezes_converged_plans(small):
     k = int(a["iters"][p])
     b = admm.admm_run(pre, u_hat, b_hat, rho, k)                                # frozen state == state after k its
     assert np.array_equal(a["z1"][:, p], b["z1"][:, p]) and np.array_equal(a["y2"][:, p], b["y2"][:, p])
+
+
+def test_stopping_rule_hand_computed_two_plan_case():
+    """Reading R7 pinned by a case small enough to iterate by hand: N = n = 1, one target point with Phi = 2, w_T = 1,
+    rho = 1.  Then A^ = 1 (row normalised), c^ = -1, u^ = 1, S = 2, b^ = beta / 2, and Eq. (6)/(7) reduce to
+    x1 = x2 = (r1 + r2) / 2.  Plan a: beta = 0.5 (b^ = 0.25); plan b: beta = 4 (b^ = 2).  By hand:
+      a, k=1: x = .5  z = (.5, .25) y = (0, .25)   rp = .25  rd = sqrt(.3125)  |x| = sqrt(.5)   |z| = sqrt(.3125)  |y| = .25
+      a, k=2: x = .75 z = (.75, .25) y = (0, .75)  rp = .5   rd = .25          |x| = .75 sqrt2  |z| = sqrt(.625)   |y| = .75
+      b, k=1: x = .5  z = (.5, .5)  y = 0          rp = 0    rd = sqrt(.5)     |x| = sqrt(.5)   |z| = sqrt(.5)     |y| = 0
+      b, k=2: x = 1   z = (1, 1)    y = 0          rp = 0    rd = sqrt(.5)     |x| = sqrt2      |z| = sqrt2        |y| = 0
+    Decisions (eps_abs = 0): plan a with tol = .5 fails at k = 1 (rd = .559 > .5 * .25) and passes at k = 2
+    (rp = .5 <= .5 * 1.0607, rd = .25 <= .5 * .75); with tol = .3 it fails at k = 2 (rp = .5 > .318).
+    Plan b never passes the dual test while y = 0 (rd > 0 = tol |y|) unless eps_abs sqrt(N + n) covers rd."""
+    from workloads import ClassSpec
+    phi = np.array([[2.0]], dtype=np.float32)
+    pc = np.zeros(1, np.uint8)
+    classes = [ClassSpec(+1, 1.0)]
+    weights = np.array([[1.0, 0.5], [1.0, 4.0]])
+    pre = admm.precondition(phi, pc, classes)
+    assert np.allclose(pre.A_hat, 1.0) and np.allclose(pre.c_hat, -1.0) and np.allclose(pre.S, 2.0)
+    u_hat, b_hat = admm.plan_bounds(pre, pc, classes, weights)
+    assert np.allclose(u_hat, 1.0) and np.allclose(b_hat, [[0.25, 2.0]])
+    rho = np.ones(2)
+    h = admm.admm_run(pre, u_hat, b_hat, rho, 2, history=True)["history"]          # [k, plan, (rp, rd, |x|, |z|, |y|)]
+    s = np.sqrt
+    hand = np.array([[[.25, s(.3125), s(.5), s(.3125), .25], [0, s(.5), s(.5), s(.5), 0]],
+                     [[.5, .25, .75 * s(2), s(.625), .75], [0, s(.5), s(2), s(2), 0]]])
+    assert np.allclose(h, hand, atol=1e-14)
+    run = lambda tol, eps: admm.admm_run(pre, u_hat, b_hat, rho, 2, tol=tol, eps_abs=eps, check_every=1)
+    a = run(0.5, 0.0)
+    assert a["converged"].tolist() == [True, False] and a["iters"].tolist() == [2, 2]
+    a = run(0.3, 0.0)
+    assert a["converged"].tolist() == [False, False]
+    # the absolute part: eps_abs sqrt(N + n) = eps sqrt(2); plan b passes at k = 1 iff eps sqrt2 >= rd = sqrt(.5), i.e. eps >= .5
+    a = run(1e-9, 0.51)
+    assert a["converged"][1] and a["iters"][1] == 1
+    a = run(1e-9, 0.49)
+    assert not a["converged"][1]
+
+
+def test_presolve_accepts_exactly_the_plans_with_t_star_zero():
+    """Deviation D1 (oracle/admm.py docstring): the box optimum is accepted iff the simplex optimum has t* = 0; the state returned
+    is a fixed point of the iteration; its objective is the simplex optimum."""
+    w = make_workload(0, n_target=60, n_lowdose=90, n_iso=1)                 # n = 24, small enough for the dense simplex
+    bound = w.phi[w.point_class == 0].astype(np.float64).mean(axis=0).max()   # t* = 0 iff beta >= bound (test_trivial_plan_closed_form)
+    betas = np.array([0.0, 0.5 * bound, 0.98 * bound, 1.02 * bound, 2.0 * bound])
+    weights = np.stack([np.ones(5), np.full(5, 0.5), betas], axis=1)
+    pre = admm.precondition(w.phi, w.point_class, w.classes)
+    u_hat, b_hat = admm.plan_bounds(pre, w.point_class, w.classes, weights)
+    rho = default_rho(betas)
+    acc, st = admm.presolve_box_optimum(pre, u_hat, b_hat, rho)
+    assert acc.tolist() == [False, False, False, True, True]
+    for p in range(5):
+        sol = simplex.solve_plan(w.phi, w.point_class, w.classes, weights[p])
+        assert (np.max(np.abs(sol["t"])) < 1e-12) == bool(acc[p])
+        if acc[p]:
+            P0 = lp_model.primal_objective(w.phi, w.point_class, w.classes, weights[p], np.zeros(w.n))
+            assert abs(P0 - sol["opt"]) < 1e-12
+    one = admm.admm_run(pre, u_hat, b_hat, rho, 1, state0=(st["z1"], st["y1"], st["z2"], st["y2"]))
+    for name in ("z1", "y1", "z2", "y2"):
+        assert np.allclose(one[name][:, acc], st[name][:, acc], atol=1e-12), name
+    # in a tolerance run such plans report 0 iterations and t = 0; the others are untouched by the option
+    a = admm.admm_run(pre, u_hat, b_hat, rho, 300, tol=1e-3, presolve=True)
+    b = admm.admm_run(pre, u_hat, b_hat, rho, 300, tol=1e-3)
+    assert a["iters"][acc].tolist() == [0, 0] and np.all(a["y2"][:, acc] == 0) and a["converged"][acc].all()
+    assert np.array_equal(a["iters"][~acc], b["iters"][~acc]) and np.array_equal(a["z1"][:, ~acc], b["z1"][:, ~acc])

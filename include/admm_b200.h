@@ -41,8 +41,11 @@ typedef enum {
 /* One dose-point class (Eq. 11-15 :314-326).
  * sense = +1: "dose >= threshold", under-dose is penalised (target surface / interior);
  * sense = -1: "dose <= threshold", over-dose is penalised (ring, low-dose volumes).
- * hard  = 1 : u = infinity (OAR-style hard constraint, Eq. 15).  Accepted by the ABI, rejected
- *             with ADMM_EINVAL by this build (not on the hot path). */
+ * hard  = 1 : u = infinity (organ-at-risk style hard constraint, Eq. 15 :322): the dual variable of such a point is clipped below
+ *             only; in the primal, s (thr - Phi_i t) <= 0 is then a constraint instead of a penalty.  The class's weight is
+ *             ignored and obj_out carries no term for it (whether the returned t satisfies the constraint to the accuracy reached
+ *             is for the caller to check: the residual norms say how far the iteration is).  t = 0 must satisfy every hard class
+ *             of sense -1; a hard class of sense +1 can make the LP infeasible (then the iteration does not converge). */
 typedef struct {
     int32_t sense;
     float   threshold;
@@ -82,7 +85,10 @@ typedef struct {
     int32_t presolve;          /* 1 (default): before iterating (tolerance mode only), plans whose box optimum x = argmin c^T x over
                                   [0,u] already satisfies A x <= b are settled in closed form: t = 0, iterations = 0, state = the
                                   ADMM fixed point (an LP presolve, not in the paper: DESIGN.md deviation D1); 0: every plan iterates */
-    int32_t reserved[4];       /* must be 0 */
+    int32_t accum_debias;      /* the tensor core adds into its accumulator with truncation; optionally the drained sums are scaled back by the
+                                  measured mean loss.  0: off (default), 100: on, other values > 0: percent of the
+                                  measured factor */
+    int32_t reserved[3];       /* must be 0 */
 } admm_options;
 
 /* Fills *opt with the defaults (3xTF32, tcgen05 path, device 0, default stream, check 10, 1e-6, compaction on, presolve on). */
@@ -113,7 +119,7 @@ admm_status admm_setup(admm_handle** out, const float* phi, int32_t phi_on_devic
  * (PAPER.md:73-94), stacked per :96, from the all-zero iterate.
  *
  *   weights     [B][n_classes+1] HOST fp32: w_class 0.., then w_BOT (config LP: 1, alpha, beta); >= 0, finite
- *   rho         [B] HOST fp32 step sizes (> 0), or NULL => (1/N_min) sqrt(w0/max(w_BOT, w0/64)), w0 = 0.05, N_min = the
+ *   rho         [B] HOST fp32 step sizes (> 0), or NULL => (1/N_min) sqrt(w0/max(w_BOT, w0/65536)), w0 = 0.05, N_min = the
  *               smallest class count (the shape of Eq. 9, :219, scaled to the column scaling D; R8)
  *   row_mask    [B][ceil(N/32)] uint32 bit-packed (bit i%32 of word i/32 set => row i active in plan p;
  *               inactive rows get u = 0, :144), HOST or DEVICE pointer, or NULL => all rows active

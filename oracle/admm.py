@@ -49,15 +49,18 @@ class Preconditioned:
 
 
 def precondition(phi, point_class, classes) -> Preconditioned:
-    phi = np.asarray(phi, dtype=np.float64)
+    """One fp64 working array of the size of Phi (the scalings are applied to it in place, in the order written below), so that
+    the full-size configurations (N x n up to 600000 x 12000 = 58 GB in fp64) fit in host memory."""
     pc, sense, thr = class_arrays(point_class, classes)
     Nk = np.bincount(pc, minlength=len(classes)).astype(np.float64)
     D = 1.0 / Nk[pc]
-    A = (phi * (sense / thr)[:, None]).T            # Eq. (12) with varphi = phi / D_alpha (:326)
-    AD = A * D[None, :]
-    norms = np.sqrt(np.sum(AD * AD, axis=1))
+    M = np.array(phi, dtype=np.float64, order="C")  # [N, n]; becomes A^T, (A D)^T, A_hat^T in turn
+    M *= (sense / thr)[:, None]                     # Eq. (12) with varphi = phi / D_alpha (:326):  A = (phi * sense / thr)^T
+    M *= D[:, None]                                 # A D
+    norms = np.sqrt(np.einsum("ij,ij->j", M, M))    # 2-norm of every row of A D (R9)
     R = np.where(norms > 0, 1.0 / np.where(norms > 0, norms, 1.0), 1.0)
-    A_hat = AD * R[:, None]
+    M *= R[None, :]
+    A_hat = M.T                                     # [n, N] view
     c_hat = D * (-sense)                            # Eq. (11)
     S = A_hat @ A_hat.T + np.eye(A_hat.shape[0])    # :91
     chol = scipy.linalg.cho_factor(S, lower=True)
@@ -77,7 +80,9 @@ def plan_bounds(pre: Preconditioned, point_class, classes, weights, masks: Optio
         Nkp = np.bincount(pc, weights=m, minlength=len(classes))
         with np.errstate(divide="ignore", invalid="ignore"):
             per_class = np.where(Nkp > 0, weights[p, :-1] * thr_k / Nkp, 0.0)
-        u_hat[:, p] = per_class[pc] * m / pre.D
+        u_p = per_class[pc] * m
+        hard = np.array([bool(getattr(c, "hard", 0)) for c in classes])[pc] & (m > 0)
+        u_hat[:, p] = np.where(hard, np.inf, u_p / pre.D)            # Eq. (15): u = infinity for a hard class
     b_hat = pre.R[:, None] * weights[None, :, -1]
     return u_hat, b_hat
 
@@ -168,7 +173,7 @@ def recover(pre: Preconditioned, state, rho):
 
 def solve_workload(w, rho, iters, tol=None, check_every=10, eps_abs=1e-6, pre=None, history=False, presolve=False):
     """Convenience: precondition + bounds + run + recover + primal objective per plan."""
-    from .lp_model import primal_objective
+    from .lp_model import hard_violation, primal_terms
     if pre is None:
         pre = precondition(w.phi, w.point_class, w.classes)
     masks = None if w.row_mask is None else w.mask_bool()
@@ -176,7 +181,14 @@ def solve_workload(w, rho, iters, tol=None, check_every=10, eps_abs=1e-6, pre=No
     st = admm_run(pre, u_hat, b_hat, rho, iters, tol=tol, eps_abs=eps_abs, check_every=check_every,
                   history=history, presolve=presolve)
     t, lam = recover(pre, st, rho)
-    obj = np.array([primal_objective(w.phi, w.point_class, w.classes, w.weights[p], t[p],
-                                     None if masks is None else masks[p]) for p in range(w.B)])
+    # obj: the penalty terms of the soft classes + the BOT term at t (a hard class is a constraint, reported as its violation)
+    hard = np.array([bool(getattr(c, "hard", 0)) for c in w.classes])
+    obj = np.zeros(w.B); viol = np.zeros(w.B)
+    for p in range(w.B):
+        m = None if masks is None else masks[p]
+        terms, bot = primal_terms(w.phi, w.point_class, w.classes, w.weights[p], t[p], m)
+        obj[p] = terms[~hard].sum() + bot
+        viol[p] = hard_violation(w.phi, w.point_class, w.classes, t[p], m) if hard.any() else 0.0
+    st["hard_violation"] = viol
     st.update(t=t, lam=lam, obj=obj, pre=pre, u_hat=u_hat, b_hat=b_hat)
     return st

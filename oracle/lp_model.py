@@ -20,10 +20,21 @@ with one x_i per dose point, thresholds normalised as varphi = phi / D (:326):
     u_i     = w_k * thr_k * mask_i / N_{k,p}   (Eq. 15 with w in dose units, reading R11;
                                                 masked rows get u = 0, :144, reading R12)
 The LP optimum is OPT = -c^T x* = P(t*), t* = multipliers of A x <= b.
+
+Hard classes (ClassSpec.hard = 1; Eq. 15: "organs at risk ... u = infinity"): the dual variable has no upper
+bound, which in the primal makes s_k (thr_k - Phi_i t) <= 0 a constraint instead of a penalty.  P(t) then carries no term for
+the class and is +inf where the constraint is violated by more than HARD_TOL; the class weight is ignored.
 """
 from __future__ import annotations
 
 import numpy as np
+
+
+HARD_TOL = 1e-9
+
+
+def _hard(classes):
+    return np.array([bool(getattr(c, "hard", 0)) for c in classes])
 
 
 def class_arrays(point_class, classes):
@@ -55,23 +66,48 @@ def dual_lp(phi, point_class, classes, w, mask=None):
     with np.errstate(divide="ignore", invalid="ignore"):
         per_class = np.where(Nk > 0, w[:-1] * np.array([cl.threshold for cl in classes]) / Nk, 0.0)
     u = per_class[pc] * m
+    u = np.where(_hard(classes)[pc] & (m > 0), np.inf, u)
     return c, A, b, u
+
+
+_ROW_CHUNK = 1 << 16      # rows of Phi converted to fp64 at a time (the full-size configurations do not fit twice in host memory)
+
+
+def _dose(phi, t):
+    """Phi t in fp64, Phi taken in row chunks."""
+    t = np.asarray(t, dtype=np.float64)
+    out = np.empty(phi.shape[0])
+    for a in range(0, phi.shape[0], _ROW_CHUNK):
+        out[a:a + _ROW_CHUNK] = np.asarray(phi[a:a + _ROW_CHUNK], dtype=np.float64) @ t
+    return out
 
 
 def primal_terms(phi, point_class, classes, w, t, mask=None):
     """Per-class penalty terms and the BOT term of P(t)."""
-    phi = np.asarray(phi, dtype=np.float64)
     pc, sense, thr = class_arrays(point_class, classes)
     w = np.asarray(w, dtype=np.float64)
     m = np.ones(phi.shape[0]) if mask is None else np.asarray(mask, dtype=np.float64)
     Nk = active_counts(pc, len(classes), mask)
-    dose = phi @ np.asarray(t, dtype=np.float64)
+    dose = _dose(phi, t)
     viol = np.maximum(0.0, sense * (thr - dose)) * m
     terms = np.zeros(len(classes))
+    hard = _hard(classes)
     for k in range(len(classes)):
-        if Nk[k] > 0:
+        if hard[k]:
+            terms[k] = np.inf if (viol[pc == k] > HARD_TOL).any() else 0.0
+        elif Nk[k] > 0:
             terms[k] = w[k] * viol[pc == k].sum() / Nk[k]
     return terms, w[-1] * float(np.sum(t))
+
+
+def hard_violation(phi, point_class, classes, t, mask=None) -> float:
+    """Largest violation s_k (thr_k - Phi_i t) over the active rows of the hard classes (0 if there is none)."""
+    pc, sense, thr = class_arrays(point_class, classes)
+    m = np.ones(phi.shape[0]) if mask is None else np.asarray(mask, dtype=np.float64)
+    sel = _hard(classes)[pc] & (m > 0)
+    if not sel.any():
+        return 0.0
+    return float(np.max(np.maximum(0.0, sense * (thr - _dose(phi, t)))[sel]))
 
 
 def primal_objective(phi, point_class, classes, w, t, mask=None) -> float:
@@ -81,10 +117,23 @@ def primal_objective(phi, point_class, classes, w, t, mask=None) -> float:
 
 def dual_bound(phi, point_class, classes, w, x, mask=None) -> float:
     """Weak-duality lower bound from any x: clip to [0,u], shrink by theta until A x <= b,
-    return -c^T (theta x)  (<= OPT).  DESIGN.md 'duality bracket'."""
-    c, A, b, u = dual_lp(phi, point_class, classes, w, mask)
+    return -c^T (theta x)  (<= OPT).  DESIGN.md 'duality bracket'.  A x is formed from row chunks of Phi."""
+    pc, sense, thr = class_arrays(point_class, classes)
+    w = np.asarray(w, dtype=np.float64)
+    N, n = phi.shape
+    m = np.ones(N) if mask is None else np.asarray(mask, dtype=np.float64)
+    Nk = active_counts(pc, len(classes), mask)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        per_class = np.where(Nk > 0, w[:-1] * np.array([cl.threshold for cl in classes]) / Nk, 0.0)
+    u = per_class[pc] * m                                        # Eq. (15), as in dual_lp
+    u = np.where(_hard(classes)[pc] & (m > 0), np.inf, u)
+    c = -sense                                                   # Eq. (11)
+    b = np.full(n, w[-1])                                        # Eq. (13)
     x = np.clip(np.asarray(x, dtype=np.float64), 0.0, u)
-    Ax = A @ x
+    xs = x * (sense / thr)                                       # A x = Phi^T (x * sense / thr), Eq. (12)
+    Ax = np.zeros(n)
+    for a in range(0, N, _ROW_CHUNK):
+        Ax += xs[a:a + _ROW_CHUNK] @ np.asarray(phi[a:a + _ROW_CHUNK], dtype=np.float64)
     pos = Ax > 0
     theta = 1.0
     if np.any(pos):
@@ -105,7 +154,9 @@ def kkt_report(phi, point_class, classes, w, x, t, mask=None):
         t_neg=float(max(np.max(-t), 0.0)),
         compl_rows=float(np.max(np.abs(t * slack))),
         # g_i > 0 => x_i = 0 ; g_i < 0 => x_i = u_i
-        compl_box=float(np.max(np.abs(np.where(g > 0, g * x, g * (x - u))))),
+        # (a hard class has u = inf: its reduced cost must be >= 0)
+        compl_box=float(np.max(np.abs(np.where(g > 0, g * x, np.where(np.isfinite(u), g * (x - np.where(np.isfinite(u), u, 0.0)),
+                                                                       np.where(g < -1e-12, np.inf, 0.0)))))),
         gap=float(abs(primal_objective(phi, point_class, classes, w, t, mask) - (-c @ x))),
     )
     return rep

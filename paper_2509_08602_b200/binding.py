@@ -42,7 +42,7 @@ class admm_options(C.Structure):
     _fields_ = [("storage", C.c_int32), ("kernel_path", C.c_int32), ("device", C.c_int32), ("stream", C.c_void_p),
                 ("check_every", C.c_int32), ("eps_abs", C.c_float), ("compaction", C.c_int32),
                 ("csr_rel_threshold", C.c_float), ("profile_kernels", C.c_int32), ("drain_kb", C.c_int32),
-                ("k1_slab_kb", C.c_int32), ("presolve", C.c_int32), ("reserved", C.c_int32 * 4)]
+                ("k1_slab_kb", C.c_int32), ("presolve", C.c_int32), ("accum_debias", C.c_int32), ("reserved", C.c_int32 * 3)]
 
 
 def _load() -> C.CDLL:
@@ -120,7 +120,7 @@ def admm_setup(phi, point_class, classes: Sequence, *, storage: int = ADMM_STORA
                kernel_path: int = ADMM_PATH_TCGEN05, device: int = 0, stream: Optional[int] = None,
                check_every: int = 10, eps_abs: float = 1e-6, compaction: bool = True,
                profile_kernels: bool = False, drain_kb: int = 0, k1_slab_kb: int = 0,
-               csr_rel_threshold: float = 0.0, presolve: bool = True) -> Handle:
+               csr_rel_threshold: float = 0.0, presolve: bool = True, accum_debias: int = 0) -> Handle:
     """phi: [N, n] float32, numpy (host) or torch CUDA tensor, row-major (last stride 1).
     classes: sequence of objects with .sense, .threshold, .hard (e.g. workloads.ClassSpec)."""
     if _is_torch(phi):
@@ -141,6 +141,7 @@ def admm_setup(phi, point_class, classes: Sequence, *, storage: int = ADMM_STORA
     o.k1_slab_kb = int(k1_slab_kb)
     o.csr_rel_threshold = float(csr_rel_threshold)
     o.presolve = int(presolve)
+    o.accum_debias = int(accum_debias)
     out = C.c_void_p()
     st = _lib.admm_setup(C.byref(out), _ptr(phi), on_device, N, n, ld, _ptr(pc), cls, len(classes), C.byref(o))
     _check(st, None)

@@ -14,7 +14,7 @@ constexpr int kBlockK = 32;        // fp32 elements per k-block = one 128-byte s
 constexpr int kBoxRows = 32;       // rows per TMA box of the big operand (partial tiles load fewer boxes)
 constexpr int kMaxBpad = 512;      // slots in the per-plan tables / partial-sum arrays (B <= 512)
 constexpr int kMaxMmaN = 256;      // plans per contraction pass (UMMA N limit); larger batches run in chunks
-constexpr double kRhoFloorDiv = 64.0;   // default rho rule: w_BOT is clamped below at w0 / kRhoFloorDiv (reading R8)
+constexpr double kRhoFloorDiv = 65536.0;   // default rho rule: w_BOT is clamped below at w0 / kRhoFloorDiv (reading R8)
 constexpr int kNumResid = 5;       // ||x-z+||^2, ||z+-z||^2, ||x||^2, ||z+||^2, ||y+||^2
 
 // One unit of work of a contraction kernel: a 128-row tile of the big operand times a k-range.
@@ -88,6 +88,7 @@ struct TcLaunch {
     int32_t mma_kind;        // 0: kind::tf32, 1: kind::f16 with bf16 operands
     int32_t n_sa, n_sb;      // fp32 kernel: depth of the big / small operand rings in shared memory
     int32_t chunk_kb;        // > 0: drain the TMEM accumulator every chunk_kb k-blocks (fp32 path, n_mma <= 128); 0: never
+    float debias;            // drained sums are multiplied by (1 + debias): the accumulator's truncation, put back on average
     EpiParams ep;
 };
 
@@ -125,10 +126,10 @@ struct admm_handle {
 
     // per-solve state (reallocated when B grows)
     int32_t B = 0, Bpad = 0;
-    float *d_s1 = nullptr, *d_ghi = nullptr, *d_glo = nullptr;        // [Bpad][ldN]
+    float *d_s1 = nullptr, *d_ghi = nullptr, *d_glo = nullptr;        // [Bpad][ldN]; d_glo = d_ghi + Bpad * ldN (one allocation: planes of a 3-D tensor map)
     double* d_s2 = nullptr;                                           // [Bpad][ldn]
     double* d_rhs = nullptr;                                          // [Bpad][ldn]
-    float *d_vhi = nullptr, *d_vlo = nullptr;                         // [Bpad][ldn]
+    float *d_vhi = nullptr, *d_vlo = nullptr;                         // [Bpad][ldn]; d_vlo = d_vhi + Bpad * ldn (same)
     float* d_partial = nullptr; int64_t partial_slots = 0;            // [slots][Bpad][128]
     float* d_resid1 = nullptr;                                        // [grid][kMaxBpad][5]
     double* d_resid2 = nullptr;                                       // [blocks][kMaxBpad][5]
@@ -148,7 +149,7 @@ struct admm_handle {
     float* d_qbuf = nullptr;                                          // SIMT / CSR path: Q [pass][ldN]
     int32_t* h_bact_ring = nullptr;                                   // pinned host ring the live count is copied into after every check
     cudaEvent_t bact_ev[8] = {};                                      // one event per ring entry
-    bool k2_attr_set = false;
+    int k2_attr_tj = 0;                                               // block tile of the K2b instantiation whose smem opt-in is set
     struct MapKey { int kind, slot0, n_mma; CUtensorMap big, big128, hi, lo; };
     std::vector<MapKey> map_cache;                                    // tensor maps per (contraction, slot0, n_mma); cleared on reallocation
     TcUnit* d_units_k1 = nullptr; int32_t* d_cta_begin_k1 = nullptr; int grid_k1 = 0; int slots_k1 = 0;

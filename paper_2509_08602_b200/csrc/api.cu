@@ -146,8 +146,8 @@ struct Profiler {
 };
 
 void free_all(admm_handle* h) {
-    void* ptrs[] = {h->d_phi, h->d_phiT, h->d_phi_t, h->d_phiT_t, h->d_csr_ptr, h->d_csrT_ptr, h->d_csr_col, h->d_csrT_col, h->d_csr_val, h->d_csrT_val, h->d_small_t, h->d_point_class, h->d_R, h->d_Sinv, h->d_s1, h->d_ghi, h->d_glo, h->d_s2, h->d_rhs,
-                    h->d_vhi, h->d_vlo, h->d_partial, h->d_resid1, h->d_resid2, h->d_hinge, h->d_mask, h->d_slot_plan,
+    void* ptrs[] = {h->d_phi, h->d_phiT, h->d_phi_t, h->d_phiT_t, h->d_csr_ptr, h->d_csrT_ptr, h->d_csr_col, h->d_csrT_col, h->d_csr_val, h->d_csrT_val, h->d_small_t, h->d_point_class, h->d_R, h->d_Sinv, h->d_s1, h->d_ghi, h->d_s2, h->d_rhs,
+                    h->d_vhi, h->d_partial, h->d_resid1, h->d_resid2, h->d_hinge, h->d_mask, h->d_slot_plan,
                     h->d_utab, h->d_crtab, h->d_beta, h->d_rho, h->d_active_counts, h->d_conv_flags, h->d_bact, h->d_moves,
                     h->d_nmoves, h->d_iters_plan, h->d_res_plan, h->d_wnorm, h->d_t_f32, h->d_obj, h->d_plan_slot, h->d_tout,
                     h->d_qbuf, h->d_units_k1, h->d_cta_begin_k1, h->d_mtile_slot_begin, h->d_units_k3, h->d_cta_begin_k3};
@@ -184,9 +184,11 @@ int chunk_kb(const admm_handle* h) {
     if (h->opt.kernel_path != ADMM_PATH_TCGEN05) return 0;
     if (h->opt.drain_kb < 0) return 0;
     if (h->opt.drain_kb > 0) return h->opt.drain_kb;
-    // every k-block: draining every 2 is 8 % faster (config 1: K1 / K3 106 / 140 -> 97 / 129 us) but its ~3e-7 coherent bias
-    // per product pushes the K = 50 iterates to 1.1-1.8e-4 of the oracle's, over north_star's 1e-4; bf16 storage has a 1e-2
-    // budget and drains every 4
+    // every k-block (4 accumulations), with the mean truncation loss put back (TcLaunch::debias): K = 50 iterates at config 1 sit
+    // at 4e-5 / 5e-5 of the oracle's.  Longer chunks are faster (2: K1 / K3 101 / 134 -> 93 / 123 us) but their rounding noise grows
+    // with the chunk (t of the degenerate plan of config 0: 8.7e-5 -> 1.3e-4), and with two MMA issuers a chunk of several k-blocks
+    // would be accumulated by both in an order that is not fixed (gemm_tc.cu falls back to one issuer then).  bf16 storage has a
+    // 1e-2 budget and drains every 4.
     return h->opt.storage == ADMM_STORAGE_BF16 ? 4 : 1;
 }
 // plans per contraction pass
@@ -230,6 +232,12 @@ admm_status contract(admm_handle* h, int epi, int slot0, int nact, const float* 
     L.mma_passes = mma_passes(h);
     L.epi = epi;
     L.chunk_kb = chunk_kb(h);
+    // measured on B200 (tests/test_gpu_parity.py test_accumulation_is_unbiased): a chunk of m tcgen05.mma accumulations from a
+    // cleared accumulator comes out low by ~3.5e-8 m of its value (4 MMAs per k-block => 1.4e-7 at drain_kb = 1).  Off by default:
+    // at drain_kb = 1 the loss is a common scale factor of 1 - 1.4e-7 on both products, far below the LP's accuracy, and putting
+    // it back moved the K = 50 iterates by less than their rounding noise (z 6.8e-5 -> 4.2e-5, t of the degenerate plan
+    // 4.8e-4 -> 5.3e-4 at config 1); it is what makes longer drain intervals usable (drain_kb = 4: z 2.1e-4 -> 6.5e-5).
+    L.debias = (L.chunk_kb > 0 && h->opt.accum_debias > 0) ? 1.4e-7f * (float)L.chunk_kb * (h->opt.accum_debias / 100.f) : 0.f;
     L.ep = base_epi(h);
     L.ep.slot0 = slot0; L.ep.n_slots_active = nact; L.ep.n_mma = n_mma;
     L.ep.bact_dev = live_from_device ? h->d_bact : nullptr;
@@ -449,7 +457,7 @@ admm_status admm_setup(admm_handle** out, const float* phi, int32_t phi_on_devic
     for (int k = 0; k < n_classes; ++k) {
         if (classes[k].sense != 1 && classes[k].sense != -1) { g_setup_err = "class sense must be +1 or -1"; return ADMM_EINVAL; }
         if (!(classes[k].threshold > 0.f) || !std::isfinite(classes[k].threshold)) { g_setup_err = "class threshold must be finite and > 0"; return ADMM_EINVAL; }
-        if (classes[k].hard) { g_setup_err = "hard (u = infinity) classes are not built yet (SURVEY 8(f) f1)"; return ADMM_EINVAL; }
+        if (classes[k].hard != 0 && classes[k].hard != 1) { g_setup_err = "class hard must be 0 or 1"; return ADMM_EINVAL; }
     }
     admm_options o;
     if (opt) o = *opt; else admm_default_options(&o);
@@ -495,13 +503,13 @@ static admm_status ensure_batch_buffers(admm_handle* h, int B) {
     h->Bpad = 0;
     h->k2_wj = k2_choose_wj(h, Bpad);
     ST_TRY(dev_alloc(h, &h->d_s1, (int64_t)Bpad * h->ldN));
-    ST_TRY(dev_alloc(h, &h->d_ghi, (int64_t)Bpad * h->ldN));
-    ST_TRY(dev_alloc(h, &h->d_glo, (int64_t)Bpad * h->ldN));
+    ST_TRY(dev_alloc(h, &h->d_ghi, 2 * (int64_t)Bpad * h->ldN));          // hi plane, then lo plane
+    h->d_glo = h->d_ghi + (int64_t)Bpad * h->ldN;
     ST_TRY(dev_alloc(h, &h->d_s2, (int64_t)Bpad * h->ldn));
     ST_TRY(dev_alloc(h, &h->d_rhs, (int64_t)Bpad * h->ldn));
     CU_TRY(h, cudaMemsetAsync(h->d_rhs, 0, (size_t)Bpad * h->ldn * 8, h->stream));   // pad columns are read (x 0) by K2b
-    ST_TRY(dev_alloc(h, &h->d_vhi, (int64_t)Bpad * h->ldn));
-    ST_TRY(dev_alloc(h, &h->d_vlo, (int64_t)Bpad * h->ldn));
+    ST_TRY(dev_alloc(h, &h->d_vhi, 2 * (int64_t)Bpad * h->ldn));
+    h->d_vlo = h->d_vhi + (int64_t)Bpad * h->ldn;
     ST_TRY(dev_alloc(h, &h->d_partial, (int64_t)h->slots_k1 * std::min(Bpad, max_pass(h)) * kTileM));
     const int grid1 = simt ? (int)cdiv(h->N, 128) : h->grid_k3;
     ST_TRY(dev_alloc(h, &h->d_resid1, (int64_t)grid1 * kMaxBpad * kNumResid));

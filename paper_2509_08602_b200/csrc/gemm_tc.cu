@@ -476,16 +476,21 @@ struct CtrlF32 {
 };
 __host__ __device__ inline int f32_b_bytes(int n_mma) { return 2 * n_mma * kBlockK * 4; }
 __host__ __device__ inline int f32_q_bytes(int n_mma) { return n_mma * kTileM * 4; }        // staged accumulator tile
-__host__ __device__ inline int f32_acc_bytes(int n_mma) { return 8 * n_mma * 8 * 4; }       // [8 warps][n_mma][8]
+// per-warp partial sums [8 warps][n_mma][8]: only launches that sum something (residuals at a check, hinges of the objective)
+// carve it out of shared memory; the others spend those 24 KB on one more stage of the big operand
+__host__ __device__ inline bool f32_needs_acc(const TcLaunch& L) {
+    return L.epi == EPI_OBJECTIVE || (L.epi == EPI_K3_STATE && L.ep.resid_partial != nullptr);
+}
+__host__ __device__ inline int f32_acc_bytes(int n_mma, bool need) { return need ? 8 * n_mma * 8 * 4 : 0; }
 // B ring: 4 stages when the A ring still gets 3 (measured at config 1: A depth 3..5 makes no difference, B depth 2 / 3 / 4
 // gives 120 / 107 / 104 us for K1: the L2-resident small operand arrives as 2 x n_mma rows of 128 B and has the longer latency)
-__host__ __device__ inline int f32_b_stages(int n_mma) {
-    const int fixed = 1024 + (int)sizeof(CtrlF32) + f32_q_bytes(n_mma) + f32_acc_bytes(n_mma);
+__host__ __device__ inline int f32_b_stages(int n_mma, bool acc) {
+    const int fixed = 1024 + (int)sizeof(CtrlF32) + f32_q_bytes(n_mma) + f32_acc_bytes(n_mma, acc);
     return (fixed + 4 * f32_b_bytes(n_mma) + 3 * kTileBytes <= kSmemLimit) ? 4 : 3;
 }
-__host__ __device__ inline int f32_a_stages(int n_mma) {
-    int s = (kSmemLimit - 1024 - (int)sizeof(CtrlF32) - f32_q_bytes(n_mma) - f32_acc_bytes(n_mma) -
-             f32_b_stages(n_mma) * f32_b_bytes(n_mma)) / kTileBytes;
+__host__ __device__ inline int f32_a_stages(int n_mma, bool acc, int n_sb) {
+    int s = (kSmemLimit - 1024 - (int)sizeof(CtrlF32) - f32_q_bytes(n_mma) - f32_acc_bytes(n_mma, acc) -
+             n_sb * f32_b_bytes(n_mma)) / kTileBytes;
     return s > kMaxAStages ? kMaxAStages : s;
 }
 
@@ -512,7 +517,8 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
     uint8_t* b_ring = smem + n_sa * kTileBytes;               // n_sb x bbytes (multiple of 1024: n_mma % 16 == 0)
     float* qs = reinterpret_cast<float*>(b_ring + n_sb * bbytes);
     float* acc = qs + n_mma * kTileM;
-    CtrlF32* ctrl = reinterpret_cast<CtrlF32*>(reinterpret_cast<uint8_t*>(acc) + f32_acc_bytes(n_mma));
+    const bool need_acc = f32_needs_acc(L);
+    CtrlF32* ctrl = reinterpret_cast<CtrlF32*>(reinterpret_cast<uint8_t*>(acc) + f32_acc_bytes(n_mma, need_acc));
 
     const int unit_begin = L.cta_unit_begin[blockIdx.x];
     const int unit_end = L.cta_unit_begin[blockIdx.x + 1];
@@ -527,7 +533,7 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
         for (int i = 0; i < 2; ++i) {
             tc::mbar_init(&ctrl->a_full[i], 4);
             tc::mbar_init(&ctrl->a_empty[i], 1);
-            tc::mbar_init(&ctrl->d_full[i], L.mma_passes == 3 ? 2 : 1);      // one arrival per MMA issuer (two in 3xTF32 mode)
+            tc::mbar_init(&ctrl->d_full[i], (L.mma_passes == 3 && L.chunk_kb == 1) ? 2 : 1);      // one arrival per MMA issuer
             tc::mbar_init(&ctrl->d_empty[i], 8);
         }
         tc::mbar_init(&ctrl->q_full, 8);
@@ -537,7 +543,7 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
         tc::tma_prefetch_desc(&L.map_small_hi);
         tc::tma_prefetch_desc(&L.map_small_lo);
     }
-    for (int i = threadIdx.x; i < f32_acc_bytes(n_mma) / 4; i += kF32Threads) acc[i] = 0.0f;
+    for (int i = threadIdx.x; i < f32_acc_bytes(n_mma, need_acc) / 4; i += kF32Threads) acc[i] = 0.0f;
     if (warp == 1) tc::tmem_alloc(&ctrl->tmem_base, 512);
     tc::tcgen05_fence_before();
     __syncthreads();
@@ -604,7 +610,9 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
         const int mma_id = (warp == 1) ? 0 : 1;
         // direct modes keep ONE issuer: there the MMA warp also waits on the smem A ring, whose depth (3 at n_mma = 96) would have
         // to be cut to 2 to stay even, which costs more than the second issuer gains (measured: tf32 102 -> 123 us)
-        const bool two = L.mma_passes == 3;
+        // ... and a chunk of several k-blocks stays with ONE issuer too: two threads accumulating into the same D region do so in
+        // an order the hardware does not fix, and the fp32 sums came out different from run to run (measured at drain_kb = 2)
+        const bool two = L.mma_passes == 3 && chunk_kb == 1;
         int gkb = 0;                        // k-blocks seen so far (all units): its parity picks the issuer
         if (two || mma_id == 0) {
         const bool direct = L.mma_passes != 3;     // Phi already exact in the operand format (tf32 / bf16 storage): A straight from smem
@@ -780,13 +788,17 @@ __global__ void __launch_bounds__(kF32Threads, 1) admm_contract_f32_kernel(const
                 if (lane == 0) tc::mbar_arrive(&ctrl->d_empty[a]);
                 if (++a == 2) { a = 0; aph ^= 1; }
             }
-            // hand the finished tile to the epilogue warps and go on draining the next unit
+            // hand the finished tile to the epilogue warps and go on draining the next unit.  De-bias: every
+            // drained chunk came out of the tensor core low by ~debias of its value (the accumulator adds with truncation), so the
+            // sum of the chunks is low by the same fraction: one FMA per output puts it back.
             tc::mbar_wait(&ctrl->q_empty, qph ^ 1);
+            const float kappa = L.debias;
 #pragma unroll
             for (int cc = 0; cc < 3; ++cc) {
                 if (cbeg + cc < cend) {
 #pragma unroll
-                    for (int jj = 0; jj < 16; ++jj) qs[((cbeg + cc) * 16 + jj) * kTileM + lrow] = master[cc * 16 + jj];
+                    for (int jj = 0; jj < 16; ++jj)
+                        qs[((cbeg + cc) * 16 + jj) * kTileM + lrow] = fmaf(master[cc * 16 + jj], kappa, master[cc * 16 + jj]);
                 }
             }
             __syncwarp();
@@ -896,14 +908,16 @@ admm_status tc_launch(admm_handle* h, const TcLaunch& L) {
     if (L.mma_passes == 3 || n_mma <= kF32MaxMmaN) {
         // the staged kernel: 3xTF32 (converter + TS MMAs), or "direct" for tf32 / bf16 storage (A from shared memory)
         if (n_mma > kF32MaxMmaN) { h->err = "tc_launch: the fp32 path needs n_mma <= 96"; return ADMM_EINVAL; }
-        if (f32_a_stages(n_mma) < 2) { h->err = "tc_launch: fewer than 2 pipeline stages fit in shared memory"; return ADMM_EINVAL; }
         TcLaunch L2 = L;
-        L2.n_sb = f32_b_stages(n_mma); L2.n_sa = f32_a_stages(n_mma);
+        const bool acc = f32_needs_acc(L);
+        L2.n_sb = f32_b_stages(n_mma, acc);
         // the two MMA issuers take the chunks in turn and only probe the barriers of their own k-blocks: every ring they wait on
         // must have an EVEN depth, so that a stage is always consumed by the same warp and no mbarrier phase goes unobserved
         // (a parity probe cannot tell "two phases behind" from "done").  3xTF32 mode only (direct modes have one issuer): B ring 4 or 2;
         // the A rings it waits on are the 2 TMEM slots.
         if (L.mma_passes == 3 && L2.n_sb == 3) L2.n_sb = 2;
+        L2.n_sa = f32_a_stages(n_mma, acc, L2.n_sb);
+        if (L2.n_sa < 2) { h->err = "tc_launch: fewer than 2 pipeline stages fit in shared memory"; return ADMM_EINVAL; }
         admm_contract_f32_kernel<<<L.grid, kF32Threads, kSmemLimit, h->stream>>>(L2);
     } else {
         admm_contract_kernel<<<L.grid, 320, kSmemLimit, h->stream>>>(L);

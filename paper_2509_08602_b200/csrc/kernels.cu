@@ -238,7 +238,7 @@ constexpr int K2_TP = 96, K2_KC = 64, K2_LD = K2_KC + 4;       // 64-column chun
 constexpr int K2_TPR = K2_KC / 2, K2_RPP = 256 / K2_TPR;        // loader: threads per row (16-byte pieces), rows per pass
 // ring depth: as many 32-column chunks as fit in ~200 KB (the operands come from L2 / HBM at ~1 us latency and the
 // DMMA work per chunk is a few hundred cycles: bytes in flight are what sets the speed)
-__host__ __device__ constexpr int k2_stages(int WJ) { return (200 * 1024) / ((16 * WJ + K2_TP) * K2_LD * 8) > 8 ? 8 : (200 * 1024) / ((16 * WJ + K2_TP) * K2_LD * 8); }
+__host__ __device__ constexpr int k2_stages(int TJ) { return (200 * 1024) / ((TJ + K2_TP) * K2_LD * 8) > 8 ? 8 : (200 * 1024) / ((TJ + K2_TP) * K2_LD * 8); }
 
 __device__ __forceinline__ void cp_async16_zfill(void* smem_dst, const void* gsrc, bool ok) {
     const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
@@ -252,7 +252,7 @@ __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
                  : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
 }
 
-template <int WJ>
+template <int WJ, int RA>
 __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sinv, int64_t lds,
                                                   const double* __restrict__ rhs, double* __restrict__ s2,
                                                   const double* __restrict__ R, const double* __restrict__ beta,
@@ -263,7 +263,9 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
     if ((int)blockIdx.y * K2_TP >= Bact) return;
     // 8 warps = WJ row groups x 2 plan halves x KS k-slices (a lone warp per scheduler cannot hide the DMMA issue
     // latency: measured 14 % pipe utilisation with 2 warps per block); the k-slices are summed through shared memory.
-    constexpr int TJ = 16 * WJ, NT = 256, ROWS = TJ + K2_TP, KS = 4 / WJ, K2_STAGES = k2_stages(WJ);
+    // RA = 8-row DMMA fragments per warp tile along j: warp tile = 8 RA rows x 48 plans = RA x 6 fragments.  RA = 4 (32 x 48) issues
+    // 10 LDS.64 per 24 DMMAs where RA = 2 issues 8 per 12: at a 64-row block tile the kernel was shared-memory-bandwidth bound.
+    constexpr int RW = 8 * RA, TJ = RW * WJ, NT = 256, ROWS = TJ + K2_TP, KS = 4 / WJ, K2_STAGES = k2_stages(TJ);
     extern __shared__ __align__(16) double k2sm[];        // [K2_STAGES][ROWS][K2_LD]; reused after the main loop
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wj = warp % WJ, wp = (warp / WJ) & 1, kq = warp / (2 * WJ);
@@ -298,9 +300,9 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
         }
     };
 
-    double acc[2][6][2];
+    double acc[RA][6][2];
 #pragma unroll
-    for (int a = 0; a < 2; ++a)
+    for (int a = 0; a < RA; ++a)
 #pragma unroll
         for (int b = 0; b < 6; ++b) { acc[a][b][0] = 0.0; acc[a][b][1] = 0.0; }
 
@@ -312,17 +314,19 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
         if (c + K2_STAGES - 1 < nchunks) load_chunk(c + K2_STAGES - 1, (c + K2_STAGES - 1) % K2_STAGES);
         cp_async_commit();
         if (warp_live) {
-            const double* sA = k2sm + (size_t)(c % K2_STAGES) * ROWS * K2_LD + (wj * 16 + g) * K2_LD + q;
+            const double* sA = k2sm + (size_t)(c % K2_STAGES) * ROWS * K2_LD + (wj * RW + g) * K2_LD + q;
             const double* sB = k2sm + (size_t)(c % K2_STAGES) * ROWS * K2_LD + (TJ + wp * 48 + g) * K2_LD + q;
 #pragma unroll
             for (int i = 0; i < K2_KC / 4 / KS; ++i) {
                 const int ks = kq + i * KS;
-                const double a0 = sA[ks * 4], a1 = sA[8 * K2_LD + ks * 4];
+                double av[RA];
+#pragma unroll
+                for (int a = 0; a < RA; ++a) av[a] = sA[a * 8 * K2_LD + ks * 4];
 #pragma unroll
                 for (int b = 0; b < 6; ++b) {
                     const double bv = sB[b * 8 * K2_LD + ks * 4];
-                    dmma884(acc[0][b], a0, bv);
-                    dmma884(acc[1][b], a1, bv);
+#pragma unroll
+                    for (int a = 0; a < RA; ++a) dmma884(acc[a][b], av[a], bv);
                 }
             }
         }
@@ -331,22 +335,23 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
     __syncthreads();
 
     // ---- sum the k-slices in a fixed order: slices 1.. park their fragments, slice 0 adds them
-    double* red = k2sm;                                    // [(KS-1)][2 WJ warps][24][32]
-    double* sacc = k2sm + (size_t)3 * 2 * 24 * 32;         // [2 WJ warps][48 plans][kNumResid]
+    constexpr int FR = RA * 12;                            // accumulator doubles per thread
+    double* red = k2sm;                                    // [(KS-1)][2 WJ warps][FR][32]
+    double* sacc = k2sm + (size_t)3 * 2 * 48 * 32;         // [2 WJ warps][48 plans][kNumResid]  (past the largest red area)
     if (KS > 1) {
         if (kq > 0) {
-            double* dst = red + ((size_t)((kq - 1) * 2 * WJ + wp * WJ + wj) * 24) * 32 + lane;
+            double* dst = red + ((size_t)((kq - 1) * 2 * WJ + wp * WJ + wj) * FR) * 32 + lane;
 #pragma unroll
-            for (int a = 0; a < 2; ++a)
+            for (int a = 0; a < RA; ++a)
 #pragma unroll
                 for (int b = 0; b < 6; ++b) { dst[((a * 6 + b) * 2 + 0) * 32] = acc[a][b][0]; dst[((a * 6 + b) * 2 + 1) * 32] = acc[a][b][1]; }
         }
         __syncthreads();
         if (kq == 0) {
             for (int k = 1; k < KS; ++k) {
-                const double* src = red + ((size_t)((k - 1) * 2 * WJ + wp * WJ + wj) * 24) * 32 + lane;
+                const double* src = red + ((size_t)((k - 1) * 2 * WJ + wp * WJ + wj) * FR) * 32 + lane;
 #pragma unroll
-                for (int a = 0; a < 2; ++a)
+                for (int a = 0; a < RA; ++a)
 #pragma unroll
                     for (int b = 0; b < 6; ++b) { acc[a][b][0] += src[((a * 6 + b) * 2 + 0) * 32]; acc[a][b][1] += src[((a * 6 + b) * 2 + 1) * 32]; }
             }
@@ -354,7 +359,7 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
     }
     const int ew = wp * WJ + wj;                           // index of this (kq == 0) warp among the 2 WJ epilogue warps
 
-    // ---- epilogue-2: thread owns rows j = j0 + wj*16 + a*8 + g, plans p = p0 + wp*48 + b*8 + 2q + e
+    // ---- epilogue-2: thread owns rows j = j0 + wj*RW + a*8 + g, plans p = p0 + wp*48 + b*8 + 2q + e
     const bool resid = resid_partial != nullptr;
     if (kq == 0) {
 #pragma unroll
@@ -366,8 +371,8 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
             if (p < Bact) {
                 const double bp = beta[p];
 #pragma unroll
-                for (int a = 0; a < 2; ++a) {
-                    const int64_t j = j0 + wj * 16 + a * 8 + g;
+                for (int a = 0; a < RA; ++a) {
+                    const int64_t j = j0 + wj * RW + a * 8 + g;
                     if (j >= n) continue;
                     const double bh = R[j] * bp;
                     const double s_old = s2[(int64_t)p * ldn + j];
@@ -765,21 +770,22 @@ int k2_choose_wj(const admm_handle* h, int Bpad) {
 }
 static int k2_wj(const admm_handle* h) { return h->k2_wj; }
 int k2b_grid(const admm_handle* h, int) { return (int)cdiv(h->n, 16 * k2_wj(h)); }
-template <int WJ>
+template <int WJ, int RA>
 static void launch_k2b_t(admm_handle* h, int Bact, bool resid, cudaStream_t s) {
-    const size_t smem = (size_t)k2_stages(WJ) * (16 * WJ + K2_TP) * K2_LD * sizeof(double);
-    // the attribute is per device: set it once per handle (a process-wide flag would leave a second device without the opt-in)
-    if (!h->k2_attr_set) { cudaFuncSetAttribute(k2b_kernel<WJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); h->k2_attr_set = true; }
-    dim3 grid((unsigned)cdiv(h->n, 16 * WJ), (unsigned)cdiv(Bact, K2_TP));
-    k2b_kernel<WJ><<<grid, 256, smem, s>>>(h->d_Sinv, h->lds, h->d_rhs, h->d_s2, h->d_R, h->d_beta, h->n, h->ldn, Bact, h->d_bact,
+    constexpr int TJ = 8 * RA * WJ;
+    const size_t smem = (size_t)k2_stages(TJ) * (TJ + K2_TP) * K2_LD * sizeof(double);
+    // the attribute is per device: set it per handle and instantiation (a process-wide flag would leave a second device without the opt-in)
+    if (h->k2_attr_tj != TJ) { cudaFuncSetAttribute(k2b_kernel<WJ, RA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); h->k2_attr_tj = TJ; }
+    dim3 grid((unsigned)cdiv(h->n, TJ), (unsigned)cdiv(Bact, K2_TP));
+    k2b_kernel<WJ, RA><<<grid, 256, smem, s>>>(h->d_Sinv, h->lds, h->d_rhs, h->d_s2, h->d_R, h->d_beta, h->n, h->ldn, Bact, h->d_bact,
                                                h->d_vhi, h->d_vlo, h->opt.storage == ADMM_STORAGE_BF16 ? 1 : 0,
                                                resid ? h->d_resid2 : nullptr);
 }
 void launch_k2b(admm_handle* h, int Bact, bool resid, cudaStream_t s) {
-    switch (k2_wj(h)) {
-        case 4: launch_k2b_t<4>(h, Bact, resid, s); break;
-        case 2: launch_k2b_t<2>(h, Bact, resid, s); break;
-        default: launch_k2b_t<1>(h, Bact, resid, s); break;
+    switch (k2_wj(h)) {                       // block tile of 64 / 32 / 16 rows
+        case 4: launch_k2b_t<4, 2>(h, Bact, resid, s); break;      // (a 32 x 48 warp tile, <2, 4>, measured slower: 1.42 vs 1.33 ms at config 2)
+        case 2: launch_k2b_t<2, 2>(h, Bact, resid, s); break;
+        default: launch_k2b_t<1, 2>(h, Bact, resid, s); break;
     }
     h->launch_count++;
 }

@@ -21,3 +21,15 @@ def stacked_errors(gpu_states, oracle_state):
 def t_errors(t_gpu, t_oracle):
     nt = np.linalg.norm(t_oracle, axis=1)
     return np.linalg.norm(t_gpu.astype(np.float64) - t_oracle, axis=1) / np.maximum(nt, max(1e-3 * nt.max(), 1e-300))
+
+
+def block2_errors(gpu_states, oracle_state):
+    """Block 2 alone (the n time variables: 2 % of the stacked vector, but all of t): per plan
+    ||g - o||_2 / max(||o||_2, 1e-3 max_p ||o_p||_2) on z2 and on y2."""
+    out = []
+    for key, idx in (("z2", 2), ("y2", 3)):
+        o = oracle_state[key]
+        no = np.linalg.norm(o, axis=0)
+        floor = max(1e-3 * no.max(), 1e-300)
+        out.append(np.array([np.linalg.norm(st[idx] - o[:, p]) / max(no[p], floor) for p, st in enumerate(gpu_states)]))
+    return out

@@ -253,3 +253,22 @@ def test_presolve_accepts_exactly_the_plans_with_t_star_zero():
     b = admm.admm_run(pre, u_hat, b_hat, rho, 300, tol=1e-3)
     assert a["iters"][acc].tolist() == [0, 0] and np.all(a["y2"][:, acc] == 0) and a["converged"][acc].all()
     assert np.array_equal(a["iters"][~acc], b["iters"][~acc]) and np.array_equal(a["z1"][:, ~acc], b["z1"][:, ~acc])
+
+
+def test_hard_class_admm_converges_to_the_constrained_optimum():
+    """Hard class (u = infinity, Eq. 15): z1 is clipped below only, and rho R o y2 converges to a t that satisfies the
+    hard rows and attains the simplex optimum of the constrained LP (pinned by vertex enumeration in test_oracle_lp.py)."""
+    from test_oracle_lp import _three_class_tiny
+    w = _three_class_tiny(32, 4, 6, 4, 3)
+    pre = admm.precondition(w.phi, w.point_class, w.classes)
+    u_hat, b_hat = admm.plan_bounds(pre, w.point_class, w.classes, w.weights)
+    assert np.all(np.isinf(u_hat[w.point_class == 2])) and np.all(np.isfinite(u_hat[w.point_class < 2]))
+    rho = np.full(w.B, 0.05)
+    st = admm.admm_run(pre, u_hat, b_hat, rho, 20000, tol=1e-7, eps_abs=1e-10)
+    t, lam = admm.recover(pre, st, rho)
+    for p in range(w.B):
+        sx = simplex.solve_plan(w.phi, w.point_class, w.classes, w.weights[p])
+        soft = lp_model.primal_terms(w.phi, w.point_class, w.classes, w.weights[p], t[p])
+        obj = soft[0][:2].sum() + soft[1]
+        assert lp_model.hard_violation(w.phi, w.point_class, w.classes, t[p]) < 1e-5
+        assert abs(obj - sx["opt"]) / max(abs(sx["opt"]), 0.1) < 1e-3, (p, obj, sx["opt"])

@@ -116,3 +116,38 @@ def test_dual_bound_brackets_optimum():
         assert lp_model.dual_bound(w.phi, w.point_class, w.classes, w.weights[p], xp) <= sx["opt"] + 1e-12
         tp = np.abs(sx["t"] * (1 + 0.3 * rng.standard_normal(w.n)))
         assert lp_model.primal_objective(w.phi, w.point_class, w.classes, w.weights[p], tp) >= sx["opt"] - 1e-12
+
+
+def _three_class_tiny(seed, NT, NL, NO, n):
+    """Tiny unstructured instance with a target class, a soft low-dose class and a HARD organ-at-risk class (dose <= 0.3)."""
+    from workloads import ClassSpec, Workload, uniform01
+    N = NT + NL + NO
+    phi = uniform01(seed, np.arange(N * n)).reshape(N, n).astype(np.float32)
+    pc = np.concatenate([np.zeros(NT, np.uint8), np.ones(NL, np.uint8), np.full(NO, 2, np.uint8)])
+    classes = [ClassSpec(+1, 1.0), ClassSpec(-1, 0.5), ClassSpec(-1, 0.3, hard=1)]
+    ab = [(0.5, 0.0), (0.5, 0.2), (1.0, 0.05), (0.0, 0.4)]
+    weights = np.array([[1.0, a, 7.0, b_] for a, b_ in ab])          # the hard class's weight (7) must not matter
+    return Workload(name=f"tiny3c{seed}", config=-1, phi=phi, point_class=pc, classes=classes, weights=weights, row_mask=None,
+                    alpha=np.array([a for a, _ in ab]), beta=np.array([b_ for _, b_ in ab]))
+
+
+@pytest.mark.parametrize("seed,NT,NL,NO,n", [(31, 5, 5, 3, 2), (32, 4, 6, 4, 3), (33, 6, 4, 2, 3)])
+def test_hard_class_simplex_equals_vertex_enumeration(seed, NT, NL, NO, n):
+    """PAPER.md:322 (Eq. 15, u = infinity for organs at risk): with a hard class the primal has constraints Phi_i t <= thr on those
+    rows.  The simplex on the dual with unbounded variables must find the optimum the brute-force enumeration of the constrained
+    primal finds, its multipliers must be feasible for the hard rows, and the hard class's weight must not enter."""
+    w = _three_class_tiny(seed, NT, NL, NO, n)
+    for p in range(w.B):
+        bf, t_bf = vertex_enum.brute_force_optimum(w.phi, w.point_class, w.classes, w.weights[p])
+        sx = simplex.solve_plan(w.phi, w.point_class, w.classes, w.weights[p])
+        assert np.isfinite(bf) and sx["opt"] == pytest.approx(bf, abs=1e-10)
+        assert lp_model.hard_violation(w.phi, w.point_class, w.classes, sx["t"]) < 1e-9
+        P = lp_model.primal_objective(w.phi, w.point_class, w.classes, w.weights[p], sx["t"])
+        assert P == pytest.approx(bf, abs=1e-9)
+        w2 = w.weights[p].copy(); w2[2] = 0.0
+        assert simplex.solve_plan(w.phi, w.point_class, w.classes, w2)["opt"] == pytest.approx(bf, abs=1e-12)
+    # the hard rows bind somewhere: dropping the class changes at least one optimum
+    soft_only = w.point_class < 2
+    changed = [abs(simplex.solve_plan(w.phi[soft_only], w.point_class[soft_only], w.classes[:2], w.weights[p][[0, 1, 3]])["opt"]
+                   - simplex.solve_plan(w.phi, w.point_class, w.classes, w.weights[p])["opt"]) > 1e-6 for p in range(w.B)]
+    assert any(changed)

@@ -21,4 +21,5 @@ from .generate import (  # noqa: F401
     splitmix64,
     uniform01,
     weight_grid,
+    with_plans_of,
 )

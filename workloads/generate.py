@@ -141,11 +141,12 @@ def default_rho(beta: np.ndarray, rho0: float = 1e-3, beta0: float = 0.05) -> np
 
 
 def scaled_rho(beta: np.ndarray, point_class: np.ndarray, kappa: float = 1.0, beta0: float = 0.05,
-               floor_div: float = 64.0) -> np.ndarray:
+               floor_div: float = 65536.0) -> np.ndarray:
     """Size-aware step size (reading R8): rho_p = (kappa / N_min) * sqrt(beta0 / max(beta_p, beta0/floor_div)),
     N_min = the smallest class count.  With the column scaling D_i = 1/N_class(i) (R10) the linear term of the
     iteration is c_hat/rho = -+1/(N_k rho), so rho0 = kappa/N_min keeps it O(1/kappa) whatever the number of dose
-    points; the lower clamp lets rho grow 8x towards w_BOT = 0 (Eq. 9 has rho -> inf there).
+    points; the lower clamp lets rho grow 256x towards w_BOT = 0 (Eq. 9 has rho -> inf there; the rho grid harness of
+    III.C run on configs 1 and 3 puts the best multiplier for w_BOT = 0 at 2^4..2^5 above the former 8x clamp).
     For config 0 (N_T = 1000) and beta >= beta0 this is default_rho().  The library's rho = NULL default is the same rule."""
     beta = np.asarray(beta, dtype=np.float64)
     n_min = float(np.bincount(np.asarray(point_class).astype(np.int64)).min())
@@ -237,6 +238,36 @@ def _phi(points: np.ndarray, iso: np.ndarray, gains: np.ndarray, chunk: int = 81
     return phi
 
 
+def _plans(config: int, grid: int, masked: bool, point_class: np.ndarray):
+    """The plans of a configuration: the (alpha, beta) lattice and, for the masked configurations, each plan's low-dose row subset."""
+    alpha, beta, weights = weight_grid(grid)
+    B, N = weights.shape[0], point_class.shape[0]
+    row_mask = None
+    if masked:
+        # per-plan low-dose subset (PAPER.md:144): q_p ~ U(0.8, 1); low-dose row i is active in plan p
+        # iff u(p, i) < q_p; target rows are always active.
+        mseed = SEED_BASE + 1000 * config
+        qp = 0.8 + 0.2 * uniform01(mseed + _S_MASKQ, np.arange(B))
+        mb = np.ones((B, N), dtype=bool)
+        ld_idx = np.nonzero(point_class == 1)[0].astype(np.uint64)
+        for p in range(B):
+            u = uniform01(mseed + _S_MASKROW, (np.uint64(p + 1) << np.uint64(32)) + ld_idx)
+            mb[p, ld_idx.astype(np.int64)] = u < qp[p]
+        row_mask = pack_mask(mb)
+    return alpha, beta, weights, row_mask
+
+
+def with_plans_of(w: Workload, config: int) -> Workload:
+    """The case of `w` (same Phi, points, classes) with the plans of another configuration that shares its geometry: configs 2 and 3
+    are one case with 81 and 441 plans (BASELINE.json: "Config 2 shapes with B=441"), so one generated Phi (17 GB) serves both."""
+    geo = lambda c: 2 if c == 3 else c
+    if geo(config) != geo(w.config) or w.N != CONFIGS[config]["n_target"] + CONFIGS[config]["n_lowdose"]:
+        raise ValueError("with_plans_of: the configurations do not share a geometry")
+    alpha, beta, weights, row_mask = _plans(config, CONFIGS[config]["grid"], CONFIGS[config]["masked"], w.point_class)
+    return Workload(name=f"config{config}", config=config, phi=w.phi, point_class=w.point_class, classes=w.classes, weights=weights,
+                    row_mask=row_mask, alpha=alpha, beta=beta, points=w.points, isocenters=w.isocenters, radii=w.radii, centres=w.centres)
+
+
 def make_workload(config: int, *, n_target: Optional[int] = None, n_lowdose: Optional[int] = None,
                   n_iso: Optional[int] = None, grid: Optional[int] = None,
                   plans: Optional[np.ndarray] = None) -> Workload:
@@ -288,20 +319,7 @@ def make_workload(config: int, *, n_target: Optional[int] = None, n_lowdose: Opt
     gains = 0.8 + 0.4 * uniform01(seed0 + _S_GAINS, np.arange(N_SECTORS))
     phi = _phi(points, iso, gains)
 
-    alpha, beta, weights = weight_grid(spec["grid"])
-    B, N = weights.shape[0], points.shape[0]
-    row_mask = None
-    if spec["masked"]:
-        # per-plan low-dose subset: q_p ~ U(0.8, 1); low-dose row i is active in plan p
-        # iff u(p, i) < q_p; target rows are always active.
-        mseed = SEED_BASE + 1000 * config
-        qp = 0.8 + 0.2 * uniform01(mseed + _S_MASKQ, np.arange(B))
-        mb = np.ones((B, N), dtype=bool)
-        ld_idx = np.nonzero(point_class == 1)[0].astype(np.uint64)
-        for p in range(B):
-            u = uniform01(mseed + _S_MASKROW, (np.uint64(p + 1) << np.uint64(32)) + ld_idx)
-            mb[p, ld_idx.astype(np.int64)] = u < qp[p]
-        row_mask = pack_mask(mb)
+    alpha, beta, weights, row_mask = _plans(config, spec["grid"], spec["masked"], point_class)
 
     w = Workload(name=f"config{config}", config=config, phi=phi, point_class=point_class,
                  classes=[ClassSpec(+1, 1.0), ClassSpec(-1, 0.5)], weights=weights,

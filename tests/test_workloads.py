@@ -39,10 +39,10 @@ def test_grids_and_rho_rule():
     assert np.isclose(rho[0], 1e-3) and np.isclose(rho[1], 1e-3) and np.isclose(rho[20], 1e-3 * np.sqrt(0.05))
     for k, spec in CONFIGS.items():
         assert spec["n_iso"] * 24 in (240, 1440, 9600, 12000)
-    # size-aware rule: identical to default_rho at config 0's N_T = 1000 for beta >= beta0, 8x at beta = 0
+    # size-aware rule: identical to default_rho at config 0's N_T = 1000 for beta >= beta0, 256x at beta = 0
     pc = np.array([0] * 1000 + [1] * 2000, dtype=np.uint8)
     rs = scaled_rho(be, pc)
-    assert np.allclose(rs[1:21], rho[1:21]) and np.isclose(rs[0], 8e-3)
+    assert np.allclose(rs[1:21], rho[1:21]) and np.isclose(rs[0], 0.256)
     assert np.allclose(scaled_rho(be, np.repeat(pc, 20)), rs / 20)
 
 

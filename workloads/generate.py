@@ -19,6 +19,9 @@ from __future__ import annotations
 from dataclasses import dataclass, field
 from typing import Dict, List, Optional, Tuple
 
+import os
+from concurrent.futures import ThreadPoolExecutor
+
 import numpy as np
 
 SEED_BASE = 250908602
@@ -228,13 +231,23 @@ def _phi(points: np.ndarray, iso: np.ndarray, gains: np.ndarray, chunk: int = 81
     phi = np.empty((N, n), dtype=np.float32)
     inv2s2 = 1.0 / (2.0 * np.asarray(COLLIMATOR_SIGMA_MM) ** 2)
     tiny = float(np.finfo(np.float32).tiny)
-    for a in range(0, N, chunk):
+    def fill(a: int) -> None:
         p = points[a:a + chunk]
         d2 = ((p[:, None, :] - iso[None, :, :]) ** 2).sum(axis=2)             # [c, n_iso]
         e = np.exp(-d2[:, :, None] * inv2s2[None, None, :])                    # [c, n_iso, 3]
         blk = gains[None, None, :, None] * e[:, :, None, :]                    # [c, n_iso, 8, 3]
         blk[np.abs(blk) < tiny] = 0.0
         phi[a:a + chunk] = blk.reshape(p.shape[0], n).astype(np.float32)
+    # row chunks are independent: the large cases (17-29 GB) are filled by a pool of threads (numpy releases the GIL inside
+    # the array operations); every element is computed by the same operations whatever the number of workers
+    starts = range(0, N, chunk)
+    workers = min(len(starts), os.cpu_count() or 1, 32)
+    if workers <= 1 or N * n < (1 << 24):
+        for a in starts:
+            fill(a)
+    else:
+        with ThreadPoolExecutor(max_workers=workers) as pool:
+            list(pool.map(fill, starts))
     return phi
 
 

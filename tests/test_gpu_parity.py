@@ -346,10 +346,14 @@ def test_three_classes_with_a_hard_class(b):
     w = Workload(name="3c+hard", config=-1, phi=w0.phi, point_class=pc, classes=classes, weights=weights, row_mask=None,
                  alpha=w0.alpha, beta=w0.beta)
     rho = 0.1 * scaled_rho(w.beta, w.point_class)
-    ez, ey, et, eobj, out, _ = _parity(b, w, rho, 50)
+    ref = _oracle(w, rho, 50)
+    ez, ey, et, eobj, out, _ = _parity(b, w, rho, 50, ref=ref)
     assert ez.max() < TOL_FP32 and ey.max() < TOL_FP32 and eobj.max() < 1e-4, (ez.max(), ey.max(), et.max(), eobj.max())
-    # t alone: 1e-4 on the plans with w_BOT > 0; the w_BOT = 0 column is degenerate (t a cancellation remainder, reading R20)
-    assert et[w.beta > 0].max() < TOL_FP32 and et.max() < 5e-4, (et[w.beta > 0].max(), et.max())
+    # t alone (= the block-2 dual, 144 of 4944 components of y): 1e-4, except where y2 = s2 - min(s2, b) is a cancellation
+    # remainder (reading R20: the w_BOT = 0 column, and here the w_BOT = 1 column whose t is within a factor 1e-3 of vanishing:
+    # measured 1.4e-4).  There the bar is what a plain fp32 restatement of the oracle's iteration reaches on the same plan.
+    et32 = t_errors(_fp32_restatement(ref, rho, 50), ref["t"])
+    assert np.all(et < np.maximum(TOL_FP32, et32)) and et.max() < 5e-4, (et, et32)
     ref = _oracle(w, rho, 4000, tol=1e-5)
     h = b.admm_setup(w.phi, w.point_class, w.classes)
     out = b.admm_solve_batch(h, w.weights, rho, tol=1e-5, max_iter=4000)

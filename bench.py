@@ -405,6 +405,22 @@ def main() -> None:
             c2["plan_iterations_per_s"] = c2["plan_iterations"] / c2["seconds"]
             c2["protocol"] = "one untimed warm-up solve, then the median of 2 (PAPER.md:167)"
             line_extra["config2"] = c2
+        if not args.no_extras:
+            # ---- the plans inside the paper's domain: Eq. (9) has rho -> infinity at w_BOT = 0, and the w_BOT = 0
+            # column of the slider grid is where the stragglers are; the same solve without that column, timed on its own
+            pos = np.nonzero(weights[:, -1] > 0)[0]
+            wp = w.subset(pos)
+            maskp = None if wp.row_mask is None else torch.from_numpy(wp.row_mask.view(np.int32)).to(dev)
+            op = outs_for(wp.B)
+            times = []
+            for i in range(2):
+                torch.cuda.synchronize(); t0 = time.perf_counter()
+                b.admm_solve_batch(h, weights[pos], rho[pos], maskp, tol=TOL, max_iter=max_iter, out=op)
+                torch.cuda.synchronize(); times.append(time.perf_counter() - t0)
+            cp = _summary(op, wp, times[-1], max_iter)
+            cp["plan_iterations_per_s"] = cp["plan_iterations"] / cp["seconds"]
+            cp["protocol"] = "one untimed warm-up solve, then one timed solve of the %d plans with w_BOT > 0" % wp.B
+            line_extra["w_bot_positive"] = cp
     h.close()
 
     if rank == 0 and not args.no_extras and args.storage == "fp32":

@@ -349,11 +349,16 @@ def test_three_classes_with_a_hard_class(b):
     ref = _oracle(w, rho, 50)
     ez, ey, et, eobj, out, _ = _parity(b, w, rho, 50, ref=ref)
     assert ez.max() < TOL_FP32 and ey.max() < TOL_FP32 and eobj.max() < 1e-4, (ez.max(), ey.max(), et.max(), eobj.max())
-    # t alone (= the block-2 dual, 144 of 4944 components of y): 1e-4, except where y2 = s2 - min(s2, b) is a cancellation
-    # remainder (reading R20: the w_BOT = 0 column, and here the w_BOT = 1 column whose t is within a factor 1e-3 of vanishing:
-    # measured 1.4e-4).  There the bar is what a plain fp32 restatement of the oracle's iteration reaches on the same plan.
-    et32 = t_errors(_fp32_restatement(ref, rho, 50), ref["t"])
-    assert np.all(et < np.maximum(TOL_FP32, et32)) and et.max() < 5e-4, (et, et32)
+    # t alone (= the block-2 dual, 144 of 4944 components of y).  Measured: 1e-5 everywhere except the w_BOT = 1 column, 1.4e-4:
+    # there t is within 1e-3 of vanishing (y2 = s2 - min(s2, b) is a small remainder) and the tensor core's accumulator truncation
+    # -- every product comes out low by ~1.4e-7, coherently -- is amplified by that cancellation; a plain fp32
+    # restatement of the oracle, whose rounding is unbiased, sits at 1e-5 on the same plans.  With the mean truncation loss put
+    # back (accum_debias = 100) the tensor path is at 1.7e-5.  Both are asserted: the default at the measured 2e-4 on that
+    # column and 1e-4 elsewhere, the de-biased mode at 1e-4 everywhere (the w_BOT = 0 column: reading R20).
+    near_zero_t = w.beta == 1.0
+    assert et[(w.beta > 0) & ~near_zero_t].max() < TOL_FP32 and et[near_zero_t].max() < 2e-4 and et.max() < 5e-4, et
+    _, _, et_db, _, _, _ = _parity(b, w, rho, 50, ref=ref, accum_debias=100)
+    assert et_db[w.beta > 0].max() < TOL_FP32, et_db
     ref = _oracle(w, rho, 4000, tol=1e-5)
     h = b.admm_setup(w.phi, w.point_class, w.classes)
     out = b.admm_solve_batch(h, w.weights, rho, tol=1e-5, max_iter=4000)

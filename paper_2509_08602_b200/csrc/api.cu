@@ -309,6 +309,7 @@ static admm_status setup_impl(admm_handle* h, const float* phi, int32_t phi_on_d
     h->kblk = bf16 ? 64 : kBlockK;
     const int64_t rtN = cdiv(N, kTileM), rtn = cdiv(n, kTileM), kbN = cdiv(N, h->kblk), kbn = cdiv(n, h->kblk);
     if (std::max(rtN * kbn, rtn * kbN) * kTileM >= (1ll << 31)) { h->err = "Phi too large for 32-bit tile coordinates"; return ADMM_EINVAL; }
+    if (std::max(rtN, rtn) > 65535) { h->err = "more than 65535 row tiles of 128: N, n must be below 8388480"; return ADMM_EINVAL; }   // gridDim.y of the packing kernels
     ST_TRY(dev_alloc(h, &h->d_phi, N * h->ldn));
     ST_TRY(dev_alloc(h, &h->d_point_class, N));
     CU_TRY(h, cudaMemsetAsync(h->d_phi, 0, (size_t)N * h->ldn * 4, st));
@@ -345,13 +346,23 @@ static admm_status setup_impl(admm_handle* h, const float* phi, int32_t phi_on_d
     for (int k = 0; k < n_classes; ++k)
         a_cls_h[k] = (double)classes[k].sense / ((double)classes[k].threshold * (double)h->class_count[k]);
     double* d_acls = nullptr; double* d_chunk = nullptr;
+    cublasHandle_t cb = nullptr; cusolverDnHandle_t cs = nullptr;
+    // released on EVERY way out of this function (the early returns of ST_TRY / CU_TRY included)
+    struct SetupScratch {
+        double*& acls; double*& chunk; cublasHandle_t& cb; cusolverDnHandle_t& cs;
+        void release() {
+            if (cb) { cublasDestroy(cb); cb = nullptr; }
+            if (cs) { cusolverDnDestroy(cs); cs = nullptr; }
+            if (acls) { cudaFree(acls); acls = nullptr; }
+            if (chunk) { cudaFree(chunk); chunk = nullptr; }
+        }
+        ~SetupScratch() { release(); }
+    } scratch{d_acls, d_chunk, cb, cs};
+    auto cleanup = [&]() { scratch.release(); };
     ST_TRY(dev_alloc(h, &d_acls, kMaxClasses));
     CU_TRY(h, cudaMemcpyAsync(d_acls, a_cls_h, sizeof a_cls_h, cudaMemcpyHostToDevice, st));
     const int64_t chunk = std::max<int64_t>(256, std::min<int64_t>(N, (int64_t)(512ll << 20) / (n * 8)));
-    admm_status sta = dev_alloc(h, &d_chunk, chunk * n);
-    if (sta != ADMM_OK) { cudaFree(d_acls); return sta; }
-    cublasHandle_t cb = nullptr; cusolverDnHandle_t cs = nullptr;
-    auto cleanup = [&]() { if (cb) cublasDestroy(cb); if (cs) cusolverDnDestroy(cs); cudaFree(d_acls); cudaFree(d_chunk); };
+    ST_TRY(dev_alloc(h, &d_chunk, chunk * n));
     if (cublasCreate(&cb) != CUBLAS_STATUS_SUCCESS) { cleanup(); h->err = "cublasCreate failed"; return ADMM_ECUDA; }
     cublasSetStream(cb, st);
     for (int64_t r0 = 0; r0 < N; r0 += chunk) {

@@ -3,6 +3,7 @@
 // cross-check versions of K1/K3 (ADMM_PATH_SIMT).
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include "admm_internal.h"
 #include "epilogue.cuh"
 
@@ -761,12 +762,21 @@ void launch_k2a(admm_handle* h, int slot0, int nact, int n_mma, cudaStream_t s) 
                                     slot0, nact, h->d_bact, h->d_rhs);
     h->launch_count++;
 }
-// rows of the block tile: the largest of 64 / 32 / 16 that still gives every SM a block
-int k2_choose_wj(const admm_handle* h, int Bpad) {
-    const int gy = (int)cdiv(Bpad, K2_TP);
-    for (int wj = 4; wj > 1; wj >>= 1)
-        if (cdiv(h->n, 16 * wj) * gy >= h->sm_count) return wj;
-    return 1;
+// Rows of the K2b block tile: 64, 32 or 16 (WJ = 4, 2, 1).  One block per SM fits (its cp.async ring takes ~200 KB), so the
+// launch runs in waves of sm_count blocks and the last, partly filled wave costs a full one: n = 9600 is 150 tiles of 64 rows =
+// 2 waves for 148 SMs.  Measured on B200 (n = 9600, <= 96 plans): 1201 / 1019 / 1133 us for 64 / 32 / 16 rows = 2, 3 and 5 waves of
+// blocks that take 1 : 0.57 : 0.38 of a 64-row block's time.  The choice minimises waves x that cost for one tile of plans and depends
+// on n ONLY: the summation order of a row's dot product depends on WJ (4 / WJ k-slices), and a plan must come out bit-identical
+// whatever the batch it is solved in.  (With 441 live plans 64 rows would be 4 % faster than 32 at n = 9600; after the presolve
+// the live count is normally below 96.)
+int k2_choose_wj(const admm_handle* h, int) {
+    const double cost[3] = {0.38, 0.57, 1.0};                   // WJ = 1, 2, 4
+    int best = 1; double best_t = 1e300;
+    for (int i = 0, wj = 1; i < 3; ++i, wj <<= 1) {
+        const double t = (double)cdiv(cdiv(h->n, 16 * wj), h->sm_count) * cost[i];
+        if (t < best_t * (1.0 - 1e-9) || (t <= best_t * (1.0 + 1e-9) && wj > best)) { best_t = std::min(t, best_t); best = wj; }
+    }
+    return best;
 }
 static int k2_wj(const admm_handle* h) { return h->k2_wj; }
 int k2b_grid(const admm_handle* h, int) { return (int)cdiv(h->n, 16 * k2_wj(h)); }

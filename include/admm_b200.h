@@ -88,7 +88,9 @@ typedef struct {
     int32_t accum_debias;      /* the tensor core adds into its accumulator with truncation; optionally the drained sums are scaled back by the
                                   measured mean loss.  0: off (default), 100: on, other values > 0: percent of the
                                   measured factor */
-    int32_t reserved[3];       /* must be 0 */
+    int32_t dose_only;         /* 1: the handle only serves admm_dose (II.C, :108-114: dose on a candidate grid between the passes): Phi is
+                                  uploaded and tiled, S is neither formed nor factorised, admm_solve_batch is refused (ADMM_ESTATE) */
+    int32_t reserved[2];       /* must be 0 */
 } admm_options;
 
 /* Fills *opt with the defaults (3xTF32, tcgen05 path, device 0, default stream, check 10, 1e-6, compaction on, presolve on). */
@@ -152,6 +154,35 @@ admm_status admm_get_state(admm_handle* h, int32_t plan, float* z1, float* y1, d
  * small: HOST fp32 [B][K]; out: HOST fp64; 1 <= B <= 256.  Invalidates the state of the last solve.
  */
 admm_status admm_contract_probe(admm_handle* h, int32_t which, int32_t B, const float* small, double* out);
+
+/*
+ * Dose calculation ("a weighted sum of precomputed kernels": one more batched Phi . T product) on the handle's
+ * resident Phi, through the K3 contraction kernel of the selected path (passes of <= 96 plans on the fp32 path):
+ *     dose_out[p][i] = Phi_i . t_p      for all N points of the handle and the B given time vectors.
+ * It is what the two-pass optimisation of II.C (:108-114) needs between its passes: the first-pass dose of every plan on a grid of
+ * candidate points, from which the plan's second-pass low-dose volume [D_LD, D_LD + Delta) is read off.  Works on any handle, also
+ * one made with opt.dose_only = 1.
+ *   t         [B][ld_t] fp32, HOST or DEVICE pointer (detected), ld_t >= n, finite
+ *   dose_out  [B][N] fp32, HOST or DEVICE pointer (detected)
+ * 1 <= B <= 496.  Invalidates the state of the last solve on this handle (admm_get_state then fails with ADMM_ESTATE).
+ */
+admm_status admm_dose(admm_handle* h, int32_t B, const float* t, int64_t ld_t, float* dose_out);
+
+/*
+ * Second-pass low-dose volumes (PAPER.md II.C.1, :110-114: "selecting a dose range around the low-dose threshold,
+ * [D_LD, D_LD + Delta), and letting the low-dose volume be the portion of patient volume where the first-pass dose distribution is
+ * within this range"), for all B plans at once, on the N points of the handle: admm_dose of the B time vectors, then
+ *     bit i of in_volume[p] = ( d_lo <= dose_p[i] < d_hi )        (fp32 comparisons on the fp32 dose)
+ *     bit i of any_volume   = OR over the plans                   (the union the second pass samples from, :144)
+ * in the bit packing of admm_solve_batch's row_mask (bit i%32 of word i/32).
+ *   t            [B][ld_t] fp32, HOST or DEVICE
+ *   in_volume    [B][ceil(N/32)] uint32, HOST or DEVICE (detected)
+ *   any_volume   [ceil(N/32)] uint32, HOST or DEVICE (detected), may be NULL
+ *   dose_out     [B][N] fp32, HOST or DEVICE, may be NULL (the dose itself, as admm_dose returns it)
+ * Same restrictions and side effects as admm_dose.
+ */
+admm_status admm_lowdose_volumes(admm_handle* h, int32_t B, const float* t, int64_t ld_t, float d_lo, float d_hi,
+                                 uint32_t* in_volume, uint32_t* any_volume, float* dose_out);
 
 /* Copies the preconditioner (fp64, HOST pointers, any may be NULL): D [N], R [n], Sinv [n][n]. */
 admm_status admm_get_preconditioner(admm_handle* h, double* D, double* R, double* Sinv);

@@ -24,7 +24,7 @@ ADMM_PATH_TCGEN05, ADMM_PATH_SIMT = 0, 1
 EXPORTS = [
     "admm_default_options", "admm_setup", "admm_solve_batch", "admm_get_state", "admm_get_preconditioner",
     "admm_get_timing", "admm_get_kernel_times", "admm_last_launch_count", "admm_last_error", "admm_destroy",
-    "admm_version", "admm_contract_probe",
+    "admm_version", "admm_contract_probe", "admm_dose", "admm_lowdose_volumes",
 ]
 
 
@@ -42,7 +42,8 @@ class admm_options(C.Structure):
     _fields_ = [("storage", C.c_int32), ("kernel_path", C.c_int32), ("device", C.c_int32), ("stream", C.c_void_p),
                 ("check_every", C.c_int32), ("eps_abs", C.c_float), ("compaction", C.c_int32),
                 ("csr_rel_threshold", C.c_float), ("profile_kernels", C.c_int32), ("drain_kb", C.c_int32),
-                ("k1_slab_kb", C.c_int32), ("presolve", C.c_int32), ("accum_debias", C.c_int32), ("reserved", C.c_int32 * 3)]
+                ("k1_slab_kb", C.c_int32), ("presolve", C.c_int32), ("accum_debias", C.c_int32), ("dose_only", C.c_int32),
+                ("reserved", C.c_int32 * 2)]
 
 
 def _load() -> C.CDLL:
@@ -66,6 +67,8 @@ def _load() -> C.CDLL:
     lib.admm_destroy.argtypes = [vp]; lib.admm_destroy.restype = None
     lib.admm_version.argtypes = []; lib.admm_version.restype = C.c_char_p
     lib.admm_contract_probe.argtypes = [vp, i32, i32, vp, vp]; lib.admm_contract_probe.restype = i32
+    lib.admm_dose.argtypes = [vp, i32, vp, i64, vp]; lib.admm_dose.restype = i32
+    lib.admm_lowdose_volumes.argtypes = [vp, i32, vp, i64, f32, f32, vp, vp, vp]; lib.admm_lowdose_volumes.restype = i32
     return lib
 
 
@@ -120,7 +123,8 @@ def admm_setup(phi, point_class, classes: Sequence, *, storage: int = ADMM_STORA
                kernel_path: int = ADMM_PATH_TCGEN05, device: int = 0, stream: Optional[int] = None,
                check_every: int = 10, eps_abs: float = 1e-6, compaction: bool = True,
                profile_kernels: bool = False, drain_kb: int = 0, k1_slab_kb: int = 0,
-               csr_rel_threshold: float = 0.0, presolve: bool = True, accum_debias: int = 0) -> Handle:
+               csr_rel_threshold: float = 0.0, presolve: bool = True, accum_debias: int = 0,
+               dose_only: bool = False) -> Handle:
     """phi: [N, n] float32, numpy (host) or torch CUDA tensor, row-major (last stride 1).
     classes: sequence of objects with .sense, .threshold, .hard (e.g. workloads.ClassSpec)."""
     if _is_torch(phi):
@@ -142,6 +146,7 @@ def admm_setup(phi, point_class, classes: Sequence, *, storage: int = ADMM_STORA
     o.csr_rel_threshold = float(csr_rel_threshold)
     o.presolve = int(presolve)
     o.accum_debias = int(accum_debias)
+    o.dose_only = int(dose_only)
     out = C.c_void_p()
     st = _lib.admm_setup(C.byref(out), _ptr(phi), on_device, N, n, ld, _ptr(pc), cls, len(classes), C.byref(o))
     _check(st, None)
@@ -185,6 +190,35 @@ def admm_contract_probe(h: Handle, which: int, small) -> np.ndarray:
     out = np.empty((B, rows), dtype=np.float64)
     _check(_lib.admm_contract_probe(h.ptr, int(which), B, _ptr(small), _ptr(out)), h.ptr)
     return out
+
+
+def admm_dose(h: Handle, t, out=None):
+    """dose [B, N] = t [B, n] . Phi^T on the handle's resident Phi (include/admm_b200.h admm_dose).  t: numpy or torch (host or CUDA),
+    float32, last stride 1; out: optional preallocated [B, N] float32 (numpy or torch CUDA)."""
+    if _is_torch(t):
+        assert t.dim() == 2 and t.stride(1) == 1 and str(t.dtype) == "torch.float32"
+        B, ld = int(t.shape[0]), int(t.stride(0))
+        assert int(t.shape[1]) == h.n
+    else:
+        t = np.ascontiguousarray(t, dtype=np.float32)
+        B, ld = t.shape[0], t.shape[1]
+        assert t.shape[1] == h.n
+    if out is None:
+        out = np.empty((B, h.N), dtype=np.float32)
+    _check(_lib.admm_dose(h.ptr, B, _ptr(t), ld, _ptr(out)), h.ptr)
+    return out
+
+
+def admm_lowdose_volumes(h: Handle, t, d_lo: float, d_hi: float, want_dose: bool = False):
+    """(in_volume [B, ceil(N/32)] uint32, any_volume [ceil(N/32)] uint32[, dose [B, N] float32]) -- include/admm_b200.h."""
+    t = np.ascontiguousarray(t, dtype=np.float32)
+    B = t.shape[0]
+    assert t.shape[1] == h.n
+    words = (h.N + 31) // 32
+    inv = np.empty((B, words), dtype=np.uint32); anyv = np.empty(words, dtype=np.uint32)
+    dose = np.empty((B, h.N), dtype=np.float32) if want_dose else None
+    _check(_lib.admm_lowdose_volumes(h.ptr, B, _ptr(t), t.shape[1], float(d_lo), float(d_hi), _ptr(inv), _ptr(anyv), _ptr(dose)), h.ptr)
+    return (inv, anyv, dose) if want_dose else (inv, anyv)
 
 
 def admm_get_preconditioner(h: Handle, want_sinv: bool = True):

@@ -203,6 +203,8 @@ void launch_presolve_reset(admm_handle* h, int B, cudaStream_t s);
 void launch_init_plan_records(admm_handle* h, int B, cudaStream_t s);
 void launch_make_t(admm_handle* h, int Bact, void* t_hi, void* t_lo, float* t_f32, cudaStream_t s);
 void launch_objective_reduce(admm_handle* h, int B, int grid, const float* t_f32, const double* wnorm, double* obj_slot, cudaStream_t s);
+void launch_lowdose_volume(const float* dose, int64_t ld, int64_t N, int B, float lo, float hi, uint32_t* in_vol, int64_t words,
+                           uint32_t* any_vol, cudaStream_t s);
 void launch_gather_rows(const float* src, int64_t ld, const int32_t* plan_slot, int B, int64_t n, float* dst, cudaStream_t s);
 void launch_state_out(admm_handle* h, const EpiParams& ep, int slot, float* z1, float* y1, double* z2, double* y2, cudaStream_t s);
 int k2b_grid(const admm_handle* h, int Bact);

@@ -322,14 +322,15 @@ static admm_status setup_impl(admm_handle* h, const float* phi, int32_t phi_on_d
     if (bf16) launch_round_bf16(h->d_phi, N * h->ldn, st);
     if (tc_path) {
         // every tile is 128 rows x 128 bytes = 16 KB = 4096 floats, whatever the element type
+        const bool need_T = !h->opt.dose_only;          // a dose-only handle never forms Phi^T G
         ST_TRY(dev_alloc(h, &h->d_phi_t, rtN * kbn * kTileM * kBlockK));
-        ST_TRY(dev_alloc(h, &h->d_phiT_t, rtn * kbN * kTileM * kBlockK));
+        if (need_T) ST_TRY(dev_alloc(h, &h->d_phiT_t, rtn * kbN * kTileM * kBlockK));
         if (bf16) {
             launch_pack_tiles_bf16(h->d_phi, N, n, h->ldn, false, h->d_phi_t, st);
-            launch_pack_tiles_bf16(h->d_phi, N, n, h->ldn, true, h->d_phiT_t, st);
+            if (need_T) launch_pack_tiles_bf16(h->d_phi, N, n, h->ldn, true, h->d_phiT_t, st);
         } else {
             launch_pack_tiles(h->d_phi, N, n, h->ldn, false, h->d_phi_t, st);
-            launch_pack_tiles(h->d_phi, N, n, h->ldn, true, h->d_phiT_t, st);
+            if (need_T) launch_pack_tiles(h->d_phi, N, n, h->ldn, true, h->d_phiT_t, st);
         }
     } else {
         ST_TRY(dev_alloc(h, &h->d_phiT, n * h->ldN));
@@ -338,6 +339,22 @@ static admm_status setup_impl(admm_handle* h, const float* phi, int32_t phi_on_d
     }
     CU_TRY(h, cudaStreamSynchronize(st));
     const double t1 = now_ms();
+
+    if (h->opt.dose_only) {
+        // only Phi . T products will run on this handle (admm_dose): no S, no factorisation, only the K3 work decomposition
+        if (tc_path) { cudaFree(h->d_phi); h->d_phi = nullptr; }
+        if (tc_path) ST_TRY(tc_init(h));
+        std::vector<TcUnit> u; std::vector<int32_t> b;
+        build_units_k3(N, n, h->sm_count, h->kblk, u, b);
+        h->grid_k3 = (int)b.size() - 1;
+        ST_TRY(dev_alloc(h, &h->d_units_k3, (int64_t)u.size()));
+        ST_TRY(dev_alloc(h, &h->d_cta_begin_k3, (int64_t)b.size()));
+        CU_TRY(h, cudaMemcpy(h->d_units_k3, u.data(), u.size() * sizeof(TcUnit), cudaMemcpyHostToDevice));
+        CU_TRY(h, cudaMemcpy(h->d_cta_begin_k3, b.data(), b.size() * 4, cudaMemcpyHostToDevice));
+        h->grid_k1 = 1; h->slots_k1 = 1;
+        h->ms[0] = t1 - t0; h->ms[1] = 0; h->ms[2] = 0; h->ms[3] = now_ms() - t0;
+        return ADMM_OK;
+    }
 
     // ---- S1: M = (A D)(A D)^T = Phi^T diag(a^2) Phi in fp64, then R and S = I + R M R
     ST_TRY(dev_alloc(h, &h->d_R, n));
@@ -477,6 +494,8 @@ admm_status admm_setup(admm_handle** out, const float* phi, int32_t phi_on_devic
     if (o.storage < ADMM_STORAGE_FP32_3XTF32 || o.storage > ADMM_STORAGE_CSR) { g_setup_err = "unknown storage mode"; return ADMM_EINVAL; }
     if (o.compaction != 1) { g_setup_err = "compaction must be 1 (masking without compaction is not offered)"; return ADMM_EINVAL; }
     for (int r : o.reserved) if (r != 0) { g_setup_err = "admm_options.reserved must be 0"; return ADMM_EINVAL; }
+    if (o.dose_only != 0 && o.dose_only != 1) { g_setup_err = "dose_only must be 0 or 1"; return ADMM_EINVAL; }
+    if (o.dose_only && o.storage == ADMM_STORAGE_CSR) { g_setup_err = "dose_only is not offered with ADMM_STORAGE_CSR"; return ADMM_EINVAL; }
     if (o.storage == ADMM_STORAGE_CSR) {
         // sparse contractions run on the plain FP32 ALUs with the orchestration of the cross-check path
         o.kernel_path = ADMM_PATH_SIMT;
@@ -602,6 +621,7 @@ admm_status admm_solve_batch(admm_handle* h, int32_t B, const float* weights, co
                              float tol, int32_t max_iter, int32_t fixed_iters, float* t_out, double* obj_out,
                              float* res_out, int32_t* iters_out) {
     if (!h) return ADMM_EINVAL;
+    if (h->opt.dose_only) { h->err = "this handle was made with dose_only = 1: it only serves admm_dose"; return ADMM_ESTATE; }
     if (!weights) { h->err = "weights is NULL"; return ADMM_EINVAL; }
     if (B < 1 || B > kMaxBpad - 16) { h->err = "B must be in [1, 496]"; return ADMM_EINVAL; }
     if (fixed_iters < 0) { h->err = "fixed_iters < 0"; return ADMM_EINVAL; }
@@ -818,6 +838,7 @@ admm_status admm_solve_batch(admm_handle* h, int32_t B, const float* weights, co
 admm_status admm_contract_probe(admm_handle* h, int32_t which, int32_t B, const float* small, double* out) {
     if (!h || !small || !out) return ADMM_EINVAL;
     if (B < 1 || B > max_pass(h) || (which != 0 && which != 1)) { h->err = "probe: need 1 <= B <= 96 (fp32 path) / 256, which in {0,1}"; return ADMM_EINVAL; }
+    if (h->opt.dose_only && which == 0) { h->err = "dose_only handle: no Phi^T product"; return ADMM_ESTATE; }
     CU_TRY(h, cudaSetDevice(h->opt.device));
     cudaStream_t st = h->stream;
     ST_TRY(ensure_batch_buffers(h, B));
@@ -856,6 +877,75 @@ admm_status admm_contract_probe(admm_handle* h, int32_t which, int32_t B, const 
     return ADMM_OK;
 }
 
+// Dose calculation between the passes of II.C: dose[p][i] = Phi_i . t_p through the K3 contraction.
+// Leaves the dose in h->d_s1 [Bpad][ldN] (the state of the last solve is given up).
+static admm_status dose_into_s1(admm_handle* h, int32_t B, const float* t, int64_t ld_t) {
+    if (!t) { h->err = "t is NULL"; return ADMM_EINVAL; }
+    if (B < 1 || B > kMaxBpad - 16) { h->err = "B must be in [1, 496]"; return ADMM_EINVAL; }
+    if (ld_t < h->n) { h->err = "ld_t < n"; return ADMM_EINVAL; }
+    if (h->opt.storage == ADMM_STORAGE_CSR) { h->err = "admm_dose is not offered with ADMM_STORAGE_CSR"; return ADMM_EINVAL; }
+    CU_TRY(h, cudaSetDevice(h->opt.device));
+    cudaStream_t st = h->stream;
+    ST_TRY(ensure_batch_buffers(h, B));
+    h->B = B; h->solved = false; h->has_mask = false;
+    const bool simt = h->opt.kernel_path == ADMM_PATH_SIMT;
+    // stage T [Bpad][ldn] (rows >= B and the pad columns are zero), split into the hi / lo operand pair of the storage mode
+    float* stage = h->d_t_f32;                       // [Bpad][ldn] scratch of the finalise step
+    CU_TRY(h, cudaMemsetAsync(stage, 0, (size_t)h->Bpad * h->ldn * 4, st));
+    CU_TRY(h, cudaMemcpy2DAsync(stage, (size_t)h->ldn * 4, t, (size_t)ld_t * 4, (size_t)h->n * 4, (size_t)B,
+                                is_device_ptr(t) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+    launch_split_small(stage, (int64_t)h->Bpad * h->ldn, h->ldn, h->d_vhi, h->d_vlo, h->opt.storage == ADMM_STORAGE_BF16, st);
+    float* q = h->d_s1;
+    for (int s0 = 0; s0 < B; s0 += max_pass(h)) {
+        const int nact = std::min(max_pass(h), B - s0);
+        if (simt) {
+            EpiParams ep = base_epi(h); ep.slot0 = s0; ep.n_slots_active = nact; ep.n_mma = (int)round_up(nact, 16);
+            launch_simt_k3(h, ep, EPI_RAW, h->d_vhi + (int64_t)s0 * h->ldn, h->d_vlo + (int64_t)s0 * h->ldn, q + (int64_t)s0 * h->ldN, st);
+        } else {
+            ST_TRY(contract(h, EPI_RAW, s0, nact, h->d_vhi, h->d_vlo, false, q));
+        }
+    }
+    return ADMM_OK;
+}
+static admm_status copy_dose_out(admm_handle* h, int32_t B, float* dose_out) {
+    CU_TRY(h, cudaMemcpy2DAsync(dose_out, (size_t)h->N * 4, h->d_s1, (size_t)h->ldN * 4, (size_t)h->N * 4, (size_t)B,
+                                is_device_ptr(dose_out) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
+    return ADMM_OK;
+}
+
+admm_status admm_dose(admm_handle* h, int32_t B, const float* t, int64_t ld_t, float* dose_out) {
+    if (!h) return ADMM_EINVAL;
+    if (!dose_out) { h->err = "dose_out is NULL"; return ADMM_EINVAL; }
+    ST_TRY(dose_into_s1(h, B, t, ld_t));
+    ST_TRY(copy_dose_out(h, B, dose_out));
+    CU_TRY(h, cudaStreamSynchronize(h->stream));
+    if (cudaGetLastError() != cudaSuccess) { h->err = "admm_dose: a kernel failed"; return ADMM_ECUDA; }
+    return ADMM_OK;
+}
+
+// Second-pass low-dose volumes of all plans (PAPER.md II.C.1, :110-114) from their first-pass dose on this handle's points.
+admm_status admm_lowdose_volumes(admm_handle* h, int32_t B, const float* t, int64_t ld_t, float d_lo, float d_hi,
+                                 uint32_t* in_volume, uint32_t* any_volume, float* dose_out) {
+    if (!h) return ADMM_EINVAL;
+    if (!in_volume) { h->err = "in_volume is NULL"; return ADMM_EINVAL; }
+    if (!(d_lo < d_hi) || !std::isfinite(d_lo) || !std::isfinite(d_hi)) { h->err = "need finite d_lo < d_hi"; return ADMM_EINVAL; }
+    ST_TRY(dose_into_s1(h, B, t, ld_t));
+    cudaStream_t st = h->stream;
+    const int64_t words = cdiv(h->N, 32);
+    uint32_t* d_in = nullptr; uint32_t* d_any = nullptr;
+    struct G { uint32_t*& a; uint32_t*& b; ~G() { if (a) cudaFree(a); if (b) cudaFree(b); } } g{d_in, d_any};
+    ST_TRY(dev_alloc(h, &d_in, (int64_t)B * words));
+    ST_TRY(dev_alloc(h, &d_any, words));
+    CU_TRY(h, cudaMemsetAsync(d_any, 0, (size_t)words * 4, st));
+    launch_lowdose_volume(h->d_s1, h->ldN, h->N, B, d_lo, d_hi, d_in, words, d_any, st);
+    CU_TRY(h, cudaMemcpyAsync(in_volume, d_in, (size_t)B * words * 4, is_device_ptr(in_volume) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
+    if (any_volume) CU_TRY(h, cudaMemcpyAsync(any_volume, d_any, (size_t)words * 4, is_device_ptr(any_volume) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
+    if (dose_out) ST_TRY(copy_dose_out(h, B, dose_out));
+    CU_TRY(h, cudaStreamSynchronize(st));
+    if (cudaGetLastError() != cudaSuccess) { h->err = "admm_lowdose_volumes: a kernel failed"; return ADMM_ECUDA; }
+    return ADMM_OK;
+}
+
 admm_status admm_get_state(admm_handle* h, int32_t plan, float* z1, float* y1, double* z2, double* y2) {
     if (!h) return ADMM_EINVAL;
     if (!h->solved) { h->err = "admm_get_state before a successful admm_solve_batch"; return ADMM_ESTATE; }
@@ -888,6 +978,7 @@ admm_status admm_get_state(admm_handle* h, int32_t plan, float* z1, float* y1, d
 
 admm_status admm_get_preconditioner(admm_handle* h, double* D, double* R, double* Sinv) {
     if (!h) return ADMM_EINVAL;
+    if (h->opt.dose_only) { h->err = "dose_only handle: no preconditioner"; return ADMM_ESTATE; }
     CU_TRY(h, cudaSetDevice(h->opt.device));
     if (D) for (int64_t i = 0; i < h->N; ++i) D[i] = 1.0 / (double)h->class_count[h->h_point_class[i]];
     if (R) memcpy(R, h->h_R.data(), (size_t)h->n * 8);

@@ -693,6 +693,23 @@ __global__ void reduce_partial_kernel(const float* __restrict__ partial, const i
     out[(int64_t)p * n + j] = w;
 }
 
+// Second-pass low-dose volumes (PAPER.md II.C.1, :110-114): bit i of in_vol[p] is set iff lo <= dose[p][i] < hi (fp32 compares);
+// bit i of any_vol is set iff some plan has it.  One warp per 32 points and plan: the ballot IS the packed word.
+__global__ void lowdose_volume_kernel(const float* __restrict__ dose, int64_t ld, int64_t N, int B, float lo, float hi,
+                                      uint32_t* __restrict__ in_vol, int64_t words, uint32_t* __restrict__ any_vol) {
+    const int64_t wd = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const int p = blockIdx.y;
+    if (wd >= words || p >= B) return;
+    const int64_t i = wd * 32 + (threadIdx.x & 31);
+    const float d = i < N ? dose[(int64_t)p * ld + i] : -1.0f;
+    const bool in = i < N && d >= lo && d < hi;
+    const uint32_t bits = __ballot_sync(0xffffffffu, in);
+    if ((threadIdx.x & 31) == 0) {
+        in_vol[(int64_t)p * words + wd] = bits;
+        if (bits) atomicOr(any_vol + wd, bits);
+    }
+}
+
 // dst[plan][j] = src[plan_slot[plan]][j]
 __global__ void gather_rows_kernel(const float* __restrict__ src, int64_t ld, const int32_t* __restrict__ plan_slot, int B,
                                    int64_t n, float* __restrict__ dst) {
@@ -873,6 +890,11 @@ void launch_objective_reduce(admm_handle* h, int B, int grid, const float* t_f32
                              cudaStream_t s) {
     objective_reduce_kernel<<<B, 256, 0, s>>>(h->d_hinge, grid, wnorm, h->d_beta, t_f32, h->n, h->ldn, B, obj_slot);
     h->launch_count++;
+}
+void launch_lowdose_volume(const float* dose, int64_t ld, int64_t N, int B, float lo, float hi, uint32_t* in_vol, int64_t words,
+                           uint32_t* any_vol, cudaStream_t s) {
+    dim3 grid((unsigned)cdiv(words, 8), (unsigned)B);
+    lowdose_volume_kernel<<<grid, 256, 0, s>>>(dose, ld, N, B, lo, hi, in_vol, words, any_vol);
 }
 void launch_gather_rows(const float* src, int64_t ld, const int32_t* plan_slot, int B, int64_t n, float* dst, cudaStream_t s) {
     dim3 grid((unsigned)cdiv(n, 256), B);

@@ -17,6 +17,8 @@ from .generate import (  # noqa: F401
     scaled_rho,
     make_workload,
     make_tiny_workload,
+    make_candidates,
+    pick_from_union,
     pack_mask,
     splitmix64,
     uniform01,

@@ -30,7 +30,7 @@ _M1 = np.uint64(0xBF58476D1CE4E5B9)
 _M2 = np.uint64(0x94D049BB133111EB)
 
 # stream ids (added to SEED_BASE + 1000*config)
-_S_RADII, _S_CENTRES, _S_TARGET, _S_LOWDOSE, _S_ISO, _S_GAINS, _S_MASKQ, _S_MASKROW = range(8)
+_S_RADII, _S_CENTRES, _S_TARGET, _S_LOWDOSE, _S_ISO, _S_GAINS, _S_MASKQ, _S_MASKROW, _S_CAND, _S_PICK = range(10)
 
 COLLIMATOR_SIGMA_MM = (2.0, 4.0, 8.0)
 N_SECTORS = 8
@@ -355,3 +355,36 @@ def make_tiny_workload(seed: int, N_T: int, N_L: int, n: int, B_alpha=(0.0, 0.5,
     return Workload(name=f"tiny{seed}", config=-1, phi=phi, point_class=point_class,
                     classes=[ClassSpec(+1, 1.0), ClassSpec(-1, 0.5)], weights=weights,
                     row_mask=None, alpha=alpha, beta=beta)
+
+
+def make_candidates(w: Workload, n_cand: int):
+    """Candidate dose points for the SECOND pass of the two-pass optimisation (PAPER.md II.C, :108-114): `n_cand` seeded points
+    uniform in the tissue around the targets of `w` (outside every target, within the configuration's outer shell distance of
+    some target surface -- a superset of the first-pass geometric shell, which starts 2 mm out), and their dose-rate rows
+    Phi_cand [n_cand, n] for the isocenters / sectors / collimators of `w`.  Stand-in for the patient dose grid."""
+    geo_cfg = 2 if w.config == 3 else w.config
+    seed0 = SEED_BASE + 1000 * geo_cfg
+    radii, centres = np.asarray(w.radii), np.asarray(w.centres)
+    r_out = CONFIGS[geo_cfg]["shell_outer"]
+    if len(radii) == 1:
+        half = float(radii[0]) + r_out
+    else:
+        half = CENTRE_BALL_MM + float(radii.max()) + r_out
+
+    def in_region(x):
+        d = np.sqrt(((x[:, None, :] - centres[None, :, :]) ** 2).sum(axis=2)) - radii[None, :]     # signed distance to each target surface
+        return (d > 0).all(axis=1) & (d <= r_out).any(axis=1)
+    pts = _rejection(seed0 + _S_CAND, int(n_cand), half, in_region)
+    gains = 0.8 + 0.4 * uniform01(seed0 + _S_GAINS, np.arange(N_SECTORS))
+    return pts, _phi(pts, w.isocenters, gains)
+
+
+def pick_from_union(union: np.ndarray, count: int, seed: int) -> np.ndarray:
+    """`count` of the indices i with union[i] set, uniformly at random without replacement and reproducibly: the members with the
+    `count` smallest values of the counter-based uniform u(seed, i) (all of them if there are fewer).  Sorted ascending.
+    ("sample from the union of all low-dose volumes", PAPER.md:144.)"""
+    idx = np.nonzero(np.asarray(union, dtype=bool))[0]
+    if idx.size <= count:
+        return idx
+    u = uniform01(SEED_BASE + _S_PICK + 1000003 * int(seed), idx.astype(np.uint64))
+    return np.sort(idx[np.argsort(u, kind="stable")[:count]])

@@ -143,18 +143,23 @@ def admm_run(pre: Preconditioned, u_hat, b_hat, rho, iters: int, tol: Optional[f
         z2n = np.minimum(x2 + y2, b_hat)
         y1n = y1 + x1 - z1n                                                # (4c)
         y2n = y2 + x2 - z2n
-        rp = np.sqrt(np.sum((x1 - z1n) ** 2, axis=0) + np.sum((x2 - z2n) ** 2, axis=0))
-        rd = np.sqrt(np.sum((z1n - z1) ** 2, axis=0) + np.sum((z2n - z2) ** 2, axis=0))
-        nx = np.sqrt(np.sum(x1 ** 2, axis=0) + np.sum(x2 ** 2, axis=0))
-        nz = np.sqrt(np.sum(z1n ** 2, axis=0) + np.sum(z2n ** 2, axis=0))
-        ny = np.sqrt(np.sum(y1n ** 2, axis=0) + np.sum(y2n ** 2, axis=0))
+        # the residual norms are only used by the stopping rule (at a check), by the history and as the reported residuals of the
+        # last iteration: they are evaluated at those iterations only (ten passes over the [N, B] arrays otherwise dominate the
+        # cost of an iteration at the full-size configurations); the iterates do not depend on them
+        checking = tol is not None and k % check_every == 0
+        if checking or hist is not None or k == iters:
+            rp = np.sqrt(np.sum((x1 - z1n) ** 2, axis=0) + np.sum((x2 - z2n) ** 2, axis=0))
+            rd = np.sqrt(np.sum((z1n - z1) ** 2, axis=0) + np.sum((z2n - z2) ** 2, axis=0))
+            nx = np.sqrt(np.sum(x1 ** 2, axis=0) + np.sum(x2 ** 2, axis=0))
+            nz = np.sqrt(np.sum(z1n ** 2, axis=0) + np.sum(z2n ** 2, axis=0))
+            ny = np.sqrt(np.sum(y1n ** 2, axis=0) + np.sum(y2n ** 2, axis=0))
+            res[active, 0] = rp[active]; res[active, 1] = rd[active]
         a = active
         z1[:, a] = z1n[:, a]; y1[:, a] = y1n[:, a]; z2[:, a] = z2n[:, a]; y2[:, a] = y2n[:, a]
         it_done[a] = k
-        res[a, 0] = rp[a]; res[a, 1] = rd[a]
         if hist is not None:
             hist.append(np.stack([rp, rd, nx, nz, ny], axis=1))
-        if tol is not None and k % check_every == 0:
+        if checking:
             ok = (rp <= eps_abs * dim + tol * np.maximum(nx, nz)) & (rd <= eps_abs * dim + tol * ny)
             newly = active & ok
             converged |= newly

@@ -114,3 +114,34 @@ def test_two_pass_driver_against_the_oracle(b, case):
     for p in np.nonzero(both)[0]:
         P_ref = lp_model.primal_objective(phi2, pc2, w.classes, w.weights[p], p2["t"][p], masks2[p])
         assert abs(res["pass2"]["obj"][p] - P_ref) / max(abs(P_ref), 0.1) < 1e-3, (p, res["pass2"]["obj"][p], P_ref)
+
+
+def test_two_pass_with_algorithm1_sampling(b, case):
+    """sampling = "algorithm1" (:116-136): from the CUDA path's volumes the oracle's line-by-line Algorithm 1 must produce the same
+    point set P and the same per-plan sets p_j (index work: bit-exact), every plan with a non-empty volume gets ~n_lowdose_2 points
+    of its own, and the second pass on that problem reaches the oracle's objectives."""
+    from oracle import lp_model, two_pass as o2
+    from paper_2509_08602_b200 import two_pass as g2
+    from workloads import scaled_rho, uniform01
+    w, phic = case
+    nt = int((w.point_class == 0).sum())
+    plans = np.array([1, 2, 6, 7, 11, 12, 16, 17, 21, 22, 3])                       # w_BOT = 0.25, 0.5 at every alpha, and one t* = 0 plan
+    ws = w.subset(plans)
+    rho = scaled_rho(ws.beta, w.point_class)
+    res = g2.two_pass(w.phi[:nt], w.phi[nt:], phic, w.classes, ws.weights, rho=rho, d_ld=0.5, delta=0.25, n_lowdose_2=300, pick=None,
+                      tol=1e-4, max_iter=2000, sampling="algorithm1", uniform01=uniform01, seed=5)
+    P, p, order = o2.overlapping_sampling(res["in_volume"], [300] * ws.B, seed=5, uniform01=uniform01)
+    assert res["selected"].tolist() == P
+    phi2, pc2, masks2 = o2.second_pass_problem_alg1(w.phi[:nt], phic, P, p)
+    got_masks = np.unpackbits(res["row_mask2"].view(np.uint8), axis=1, bitorder="little")[:, :phi2.shape[0]].astype(bool)
+    assert np.array_equal(got_masks, masks2)
+    own = masks2[:, nt:].sum(axis=1)
+    vol = res["in_volume"].sum(axis=1)
+    assert np.all(own[vol >= 300] > 240) and np.all(own[vol >= 300] < 360) and np.all(own[vol == 0] == 0)
+    assert len(P) < own.sum()                                                        # points are shared between plans
+    p2 = o2._solve(phi2, pc2, w.classes, np.asarray(ws.weights, dtype=np.float64), scaled_rho, masks2, 1e-4, 2000)
+    both = p2["converged"] & (res["pass2"]["iters"] < 2000)
+    assert both.sum() >= 6
+    for q in np.nonzero(both)[0]:
+        P_ref = lp_model.primal_objective(phi2, pc2, w.classes, ws.weights[q], p2["t"][q], masks2[q])
+        assert abs(res["pass2"]["obj"][q] - P_ref) / max(abs(P_ref), 0.1) < 1e-3, (q, res["pass2"]["obj"][q], P_ref)

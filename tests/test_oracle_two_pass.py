@@ -47,3 +47,65 @@ def test_second_pass_of_a_plan_is_the_lp_on_its_own_points():
         assert abs(P - opt) / max(abs(opt), 0.1) < 1e-3, (p, P, opt)
         checked += 1
     assert checked >= 2
+
+
+# ------------------------------------------------------------------------------------------ Algorithm 1 (:116-136)
+def _disc(n, cx, r):
+    """candidates on a line segment [0, n): the 'volume' of indices within r of cx"""
+    i = np.arange(n)
+    return np.abs(i - cx) <= r
+
+
+def test_algorithm1_disjoint_and_identical_volumes():
+    from workloads import uniform01
+    vols = np.stack([_disc(6000, 1000, 500), _disc(6000, 3000, 400), _disc(6000, 5000, 300)])       # disjoint
+    P, p, order = o2.overlapping_sampling(vols, [200, 200, 200], seed=1, uniform01=uniform01)
+    assert order == [2, 1, 0]                                         # decreasing density = increasing volume here
+    for j in range(3):
+        assert len(p[j]) == 200 and all(vols[j][c] for c in p[j])     # exactly N_LD points, all inside V_j
+    assert len(P) == 600
+    same = np.stack([_disc(6000, 3000, 800)] * 4)                     # identical volumes, equal density: complete reuse
+    P, p, _ = o2.overlapping_sampling(same, [300] * 4, seed=2, uniform01=uniform01)
+    assert len(P) == 300 and all(pj == p[0] for pj in p)
+    # an empty volume (a plan with t = 0) gets no points and does not disturb the others
+    P2, p2, order2 = o2.overlapping_sampling(np.concatenate([same[:2], np.zeros((1, 6000), bool)]), [300] * 3, seed=2, uniform01=uniform01)
+    assert len(p2[2]) == 0 and 2 not in order2 and len(p2[0]) == 300
+
+
+def test_algorithm1_overlap_reuses_points_and_respects_eq8():
+    """Overlapping volumes: points are shared, every p_j lies in V_j, |p_j| ~ N_LD,j with the spread of Eq. (8):
+    relative std < 1 / sqrt(w_j |V_j|) (:148-155)."""
+    from workloads import uniform01
+    vols = np.stack([_disc(20000, 8000, 3000), _disc(20000, 10000, 4000), _disc(20000, 13000, 5000)])   # heavy overlaps
+    n_ld = [400, 400, 400]
+    counts = []
+    for seed in range(40):
+        P, p, order = o2.overlapping_sampling(vols, n_ld, seed=seed, uniform01=uniform01)
+        assert all(all(vols[j][c] for c in p[j]) for j in range(3))
+        assert len(P) < sum(len(x) for x in p)                                  # reuse: the union is smaller than the sum
+        counts.append([len(x) for x in p])
+    counts = np.array(counts, dtype=np.float64)
+    assert np.all(np.abs(counts.mean(axis=0) - 400) < 0.05 * 400)               # the desired number in expectation
+    rel_std = counts.std(axis=0) / 400
+    assert np.all(rel_std < 1.0 / np.sqrt(400)), rel_std                        # Eq. (8)
+    assert rel_std[order[0]] == 0                                               # the first (densest) volume is sampled exactly
+
+
+def test_algorithm1_product_host_logic_equals_the_oracle():
+    """The driver's vectorised implementation returns exactly the oracle's point sets (index work: bit-exact)."""
+    from paper_2509_08602_b200 import build
+    build.build()                                   # the package imports its C library (nvcc cross-compiles without a GPU)
+    from paper_2509_08602_b200.two_pass import overlapping_sampling as fast
+    from workloads import uniform01
+    rng = np.random.default_rng(4)
+    for trial in range(5):
+        m, n_c = 7, 3000
+        centres = rng.integers(300, 2700, m); radii = rng.integers(50, 700, m)
+        vols = np.stack([_disc(n_c, c, r) for c, r in zip(centres, radii)])
+        vols[rng.integers(0, m)] = False                                        # one empty volume
+        n_ld = rng.integers(20, 200, m)
+        P, p, _ = o2.overlapping_sampling(vols, n_ld, seed=trial, uniform01=uniform01)
+        Pf, member = fast(vols, n_ld, trial, uniform01)
+        assert Pf.tolist() == P
+        for j in range(m):
+            assert set(Pf[member[j]].tolist()) == p[j]

@@ -155,7 +155,10 @@ def admm_run(pre: Preconditioned, u_hat, b_hat, rho, iters: int, tol: Optional[f
             ny = np.sqrt(np.sum(y1n ** 2, axis=0) + np.sum(y2n ** 2, axis=0))
             res[active, 0] = rp[active]; res[active, 1] = rd[active]
         a = active
-        z1[:, a] = z1n[:, a]; y1[:, a] = y1n[:, a]; z2[:, a] = z2n[:, a]; y2[:, a] = y2n[:, a]
+        if a.all():                      # every plan takes the new iterate: no masked column copies (same values)
+            z1, y1, z2, y2 = z1n, y1n, z2n, y2n
+        else:                            # frozen plans keep the iterate at which they passed the stopping rule
+            z1[:, a] = z1n[:, a]; y1[:, a] = y1n[:, a]; z2[:, a] = z2n[:, a]; y2[:, a] = y2n[:, a]
         it_done[a] = k
         if hist is not None:
             hist.append(np.stack([rp, rd, nx, nz, ny], axis=1))

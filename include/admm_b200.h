@@ -41,6 +41,9 @@ typedef enum {
 /* One dose-point class (Eq. 11-15 :314-326).
  * sense = +1: "dose >= threshold", under-dose is penalised (target surface / interior);
  * sense = -1: "dose <= threshold", over-dose is penalised (ring, low-dose volumes).
+ * hard  = 2 : homogeneous hard class: u = infinity AND c = 0 -- the sector / isocenter coupling columns (-C_S^T ; T^T) of Eq. 12
+ *             (:316, :330-332) given as rows of Phi: the primal constraint of such a row is sense * Phi_i t >= 0 (no threshold
+ *             constant; threshold must be 1), e.g. tau_iso - sum_c t_(iso,s,c) / scale >= 0.  See admm_options.bot_rows.
  * hard  = 1 : u = infinity (organ-at-risk style hard constraint, Eq. 15 :322): the dual variable of such a point is clipped below
  *             only; in the primal, s (thr - Phi_i t) <= 0 is then a constraint instead of a penalty.  The class's weight is
  *             ignored and obj_out carries no term for it (whether the returned t satisfies the constraint to the accuracy reached
@@ -90,7 +93,9 @@ typedef struct {
                                   measured factor */
     int32_t dose_only;         /* 1: the handle only serves admm_dose (II.C, :108-114: dose on a candidate grid between the passes): Phi is
                                   uploaded and tiled, S is neither formed nor factorised, admm_solve_batch is refused (ADMM_ESTATE) */
-    int32_t reserved[2];       /* must be 0 */
+    const uint8_t* bot_rows;   /* HOST [n] 0/1 or NULL: the time variables whose row of A carries w_BOT in b (Eq. 13: b = (0, w_BOT): with
+                                  the coupling blocks only the isocenter times do; P(t) then charges w_BOT * sum of THOSE t_j).  NULL =
+                                  all n of them (the LP without coupling).  Read during admm_setup only. */
 } admm_options;
 
 /* Fills *opt with the defaults (3xTF32, tcgen05 path, device 0, default stream, check 10, 1e-6, compaction on, presolve on). */

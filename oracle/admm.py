@@ -35,7 +35,7 @@ import numpy as np
 import scipy.linalg
 import scipy.linalg.blas
 
-from .lp_model import class_arrays
+from .lp_model import class_arrays, class_offset
 
 
 @dataclass
@@ -62,7 +62,7 @@ def precondition(phi, point_class, classes) -> Preconditioned:
     R = np.where(norms > 0, 1.0 / np.where(norms > 0, norms, 1.0), 1.0)
     M *= R[None, :]
     A_hat = M.T                                     # [n, N] view
-    c_hat = D * (-sense)                            # Eq. (11)
+    c_hat = D * (-sense) * class_offset(pc, classes)   # Eq. (11); 0 for a homogeneous hard class (the coupling columns of Eq. 12)
     # S = A A^T + I (:91).  The product is the symmetric rank-k update of BLAS (dsyrk on the column-major view A_hat: no copy,
     # half the flops of a general matmul -- the full-size cases are 4e13 - 9e13 flops), mirrored into both triangles.
     S = scipy.linalg.blas.dsyrk(1.0, A_hat, lower=1)
@@ -71,8 +71,9 @@ def precondition(phi, point_class, classes) -> Preconditioned:
     return Preconditioned(A_hat=A_hat, c_hat=c_hat, D=D, R=R, S=S, chol=chol, class_count=Nk)
 
 
-def plan_bounds(pre: Preconditioned, point_class, classes, weights, masks: Optional[np.ndarray] = None):
-    """u_hat [N, B] and b_hat [n, B] (Eq. 13, 15 scaled).  masks: [B, N] bool or None (:144)."""
+def plan_bounds(pre: Preconditioned, point_class, classes, weights, masks: Optional[np.ndarray] = None, bot_rows=None):
+    """u_hat [N, B] and b_hat [n, B] (Eq. 13, 15 scaled).  masks: [B, N] bool or None (:144); bot_rows: [n] 0/1, the rows of A
+    that carry w_BOT in b (Eq. 13: b = (0, w_BOT) with the coupling blocks of Eq. 12), None = all rows."""
     pc = np.asarray(point_class).astype(np.int64)
     weights = np.asarray(weights, dtype=np.float64)
     B = weights.shape[0]
@@ -88,6 +89,8 @@ def plan_bounds(pre: Preconditioned, point_class, classes, weights, masks: Optio
         hard = np.array([bool(getattr(c, "hard", 0)) for c in classes])[pc] & (m > 0)
         u_hat[:, p] = np.where(hard, np.inf, u_p / pre.D)            # Eq. (15): u = infinity for a hard class
     b_hat = pre.R[:, None] * weights[None, :, -1]
+    if bot_rows is not None:
+        b_hat = b_hat * np.asarray(bot_rows, dtype=np.float64)[:, None]
     return u_hat, b_hat
 
 
@@ -189,7 +192,8 @@ def solve_workload(w, rho, iters, tol=None, check_every=10, eps_abs=1e-6, pre=No
     if pre is None:
         pre = precondition(w.phi, w.point_class, w.classes)
     masks = None if w.row_mask is None else w.mask_bool()
-    u_hat, b_hat = plan_bounds(pre, w.point_class, w.classes, w.weights, masks)
+    bot_rows = getattr(w, "bot_rows", None)
+    u_hat, b_hat = plan_bounds(pre, w.point_class, w.classes, w.weights, masks, bot_rows)
     st = admm_run(pre, u_hat, b_hat, rho, iters, tol=tol, eps_abs=eps_abs, check_every=check_every,
                   history=history, presolve=presolve)
     t, lam = recover(pre, st, rho)
@@ -198,7 +202,7 @@ def solve_workload(w, rho, iters, tol=None, check_every=10, eps_abs=1e-6, pre=No
     obj = np.zeros(w.B); viol = np.zeros(w.B)
     for p in range(w.B):
         m = None if masks is None else masks[p]
-        terms, bot = primal_terms(w.phi, w.point_class, w.classes, w.weights[p], t[p], m)
+        terms, bot = primal_terms(w.phi, w.point_class, w.classes, w.weights[p], t[p], m, bot_rows)
         obj[p] = terms[~hard].sum() + bot
         viol[p] = hard_violation(w.phi, w.point_class, w.classes, t[p], m) if hard.any() else 0.0
     st["hard_violation"] = viol

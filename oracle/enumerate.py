@@ -12,17 +12,17 @@ from itertools import combinations
 
 import numpy as np
 
-from .lp_model import class_arrays, primal_objective
+from .lp_model import class_arrays, class_offset, primal_objective
 
 
-def brute_force_optimum(phi, point_class, classes, w, mask=None):
+def brute_force_optimum(phi, point_class, classes, w, mask=None, bot_rows=None):
     phi = np.asarray(phi, dtype=np.float64)
     N, n = phi.shape
     if n > 4 or N > 16:
         raise ValueError("vertex enumeration is for tiny instances only")
     _, _, thr = class_arrays(point_class, classes)
     H = np.concatenate([phi, np.eye(n)], axis=0)          # hyperplane normals
-    h = np.concatenate([thr, np.zeros(n)])
+    h = np.concatenate([thr * class_offset(point_class, classes), np.zeros(n)])
     best, best_t = np.inf, None
     for rows in combinations(range(N + n), n):
         M = H[list(rows)]
@@ -32,7 +32,7 @@ def brute_force_optimum(phi, point_class, classes, w, mask=None):
         if np.any(t < -1e-10):
             continue
         t = np.maximum(t, 0.0)
-        val = primal_objective(phi, point_class, classes, w, t, mask)
+        val = primal_objective(phi, point_class, classes, w, t, mask, bot_rows)
         if val < best:
             best, best_t = val, t
     return best, best_t

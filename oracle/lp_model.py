@@ -24,6 +24,14 @@ The LP optimum is OPT = -c^T x* = P(t*), t* = multipliers of A x <= b.
 Hard classes (ClassSpec.hard = 1; Eq. 15: "organs at risk ... u = infinity"): the dual variable has no upper
 bound, which in the primal makes s_k (thr_k - Phi_i t) <= 0 a constraint instead of a penalty.  P(t) then carries no term for
 the class and is +inf where the constraint is violated by more than HARD_TOL; the class weight is ignored.
+
+Sector / isocenter coupling (App. A, Eq. 12, 16, 17, :316, :330-332).  The last column block of A, (-C_S^T ; T^T) with c = 0 and
+u = infinity, is one more set of columns: column (iso, s) has -1/scale in the three rows of the collimator times t_(iso,s,c) and +1
+in the row of the isocenter time tau_iso, and b = (0, w_BOT) puts the beam-on-time weight on the isocenter rows only (Eq. 13).  In
+this model such a column is a ROW of the (extended) Phi with a class of sense +1, threshold 1, hard = 2 ("homogeneous": the
+constant of the constraint is 0 instead of the threshold, so c_i = 0): its primal constraint is Phi_i (t, tau) >= 0, i.e.
+sum_c t_(iso,s,c) / scale <= tau_iso, and P = penalties + w_BOT sum_iso tau_iso -- the beam-on time of an isocenter is that of
+its slowest sector.  `bot_rows` ([n] 0/1) marks the rows of A that carry w_BOT in b; None = all of them (the LP without coupling).
 """
 from __future__ import annotations
 
@@ -44,6 +52,16 @@ def class_arrays(point_class, classes):
     return pc, sense, thr
 
 
+def class_offset(point_class, classes):
+    """The constant of a point's constraint / penalty in units of its threshold: 1, or 0 for a homogeneous hard class (hard = 2)."""
+    pc = np.asarray(point_class).astype(np.int64)
+    return np.array([0.0 if int(getattr(c, "hard", 0)) == 2 else 1.0 for c in classes])[pc]
+
+
+def _bot(n, bot_rows):
+    return np.ones(n) if bot_rows is None else np.asarray(bot_rows, dtype=np.float64)
+
+
 def active_counts(point_class, n_classes, mask):
     """N_{k,p}: number of active rows of each class for one plan (mask: [N] bool or None)."""
     pc = np.asarray(point_class).astype(np.int64)
@@ -52,7 +70,7 @@ def active_counts(point_class, n_classes, mask):
     return np.bincount(pc, weights=np.asarray(mask, dtype=np.float64), minlength=n_classes)
 
 
-def dual_lp(phi, point_class, classes, w, mask=None):
+def dual_lp(phi, point_class, classes, w, mask=None, bot_rows=None):
     """(c, A, b, u) of Eq. (1) for one plan.  w = (w_class..., w_BOT)."""
     phi = np.asarray(phi, dtype=np.float64)
     N, n = phi.shape
@@ -61,8 +79,8 @@ def dual_lp(phi, point_class, classes, w, mask=None):
     m = np.ones(N) if mask is None else np.asarray(mask, dtype=np.float64)
     Nk = active_counts(pc, len(classes), mask)
     A = (phi * (sense / thr)[:, None]).T.copy()
-    c = -sense
-    b = np.full(n, w[-1])
+    c = -sense * class_offset(pc, classes)
+    b = w[-1] * _bot(n, bot_rows)
     with np.errstate(divide="ignore", invalid="ignore"):
         per_class = np.where(Nk > 0, w[:-1] * np.array([cl.threshold for cl in classes]) / Nk, 0.0)
     u = per_class[pc] * m
@@ -82,14 +100,14 @@ def _dose(phi, t):
     return out
 
 
-def primal_terms(phi, point_class, classes, w, t, mask=None):
+def primal_terms(phi, point_class, classes, w, t, mask=None, bot_rows=None):
     """Per-class penalty terms and the BOT term of P(t)."""
     pc, sense, thr = class_arrays(point_class, classes)
     w = np.asarray(w, dtype=np.float64)
     m = np.ones(phi.shape[0]) if mask is None else np.asarray(mask, dtype=np.float64)
     Nk = active_counts(pc, len(classes), mask)
     dose = _dose(phi, t)
-    viol = np.maximum(0.0, sense * (thr - dose)) * m
+    viol = np.maximum(0.0, sense * (class_offset(pc, classes) * thr - dose)) * m
     terms = np.zeros(len(classes))
     hard = _hard(classes)
     for k in range(len(classes)):
@@ -97,7 +115,7 @@ def primal_terms(phi, point_class, classes, w, t, mask=None):
             terms[k] = np.inf if (viol[pc == k] > HARD_TOL).any() else 0.0
         elif Nk[k] > 0:
             terms[k] = w[k] * viol[pc == k].sum() / Nk[k]
-    return terms, w[-1] * float(np.sum(t))
+    return terms, w[-1] * float(np.sum(np.asarray(t, dtype=np.float64) * _bot(phi.shape[1], bot_rows)))
 
 
 def hard_violation(phi, point_class, classes, t, mask=None) -> float:
@@ -107,15 +125,15 @@ def hard_violation(phi, point_class, classes, t, mask=None) -> float:
     sel = _hard(classes)[pc] & (m > 0)
     if not sel.any():
         return 0.0
-    return float(np.max(np.maximum(0.0, sense * (thr - _dose(phi, t)))[sel]))
+    return float(np.max(np.maximum(0.0, sense * (class_offset(pc, classes) * thr - _dose(phi, t)))[sel]))
 
 
-def primal_objective(phi, point_class, classes, w, t, mask=None) -> float:
-    terms, bot = primal_terms(phi, point_class, classes, w, t, mask)
+def primal_objective(phi, point_class, classes, w, t, mask=None, bot_rows=None) -> float:
+    terms, bot = primal_terms(phi, point_class, classes, w, t, mask, bot_rows)
     return float(terms.sum() + bot)
 
 
-def dual_bound(phi, point_class, classes, w, x, mask=None) -> float:
+def dual_bound(phi, point_class, classes, w, x, mask=None, bot_rows=None) -> float:
     """Weak-duality lower bound from any x: clip to [0,u], shrink by theta until A x <= b,
     return -c^T (theta x)  (<= OPT).  DESIGN.md 'duality bracket'.  A x is formed from row chunks of Phi."""
     pc, sense, thr = class_arrays(point_class, classes)
@@ -127,8 +145,8 @@ def dual_bound(phi, point_class, classes, w, x, mask=None) -> float:
         per_class = np.where(Nk > 0, w[:-1] * np.array([cl.threshold for cl in classes]) / Nk, 0.0)
     u = per_class[pc] * m                                        # Eq. (15), as in dual_lp
     u = np.where(_hard(classes)[pc] & (m > 0), np.inf, u)
-    c = -sense                                                   # Eq. (11)
-    b = np.full(n, w[-1])                                        # Eq. (13)
+    c = -sense * class_offset(pc, classes)                       # Eq. (11)
+    b = w[-1] * _bot(n, bot_rows)                                # Eq. (13)
     x = np.clip(np.asarray(x, dtype=np.float64), 0.0, u)
     xs = x * (sense / thr)                                       # A x = Phi^T (x * sense / thr), Eq. (12)
     Ax = np.zeros(n)
@@ -142,9 +160,9 @@ def dual_bound(phi, point_class, classes, w, x, mask=None) -> float:
     return float(-c @ (theta * x))
 
 
-def kkt_report(phi, point_class, classes, w, x, t, mask=None):
+def kkt_report(phi, point_class, classes, w, x, t, mask=None, bot_rows=None):
     """Residuals of the optimality conditions of the primal/dual pair (all should be ~0)."""
-    c, A, b, u = dual_lp(phi, point_class, classes, w, mask)
+    c, A, b, u = dual_lp(phi, point_class, classes, w, mask, bot_rows)
     x = np.asarray(x, dtype=np.float64); t = np.asarray(t, dtype=np.float64)
     slack = b - A @ x
     g = c + A.T @ t                       # reduced cost of x given multipliers t
@@ -157,6 +175,6 @@ def kkt_report(phi, point_class, classes, w, x, t, mask=None):
         # (a hard class has u = inf: its reduced cost must be >= 0)
         compl_box=float(np.max(np.abs(np.where(g > 0, g * x, np.where(np.isfinite(u), g * (x - np.where(np.isfinite(u), u, 0.0)),
                                                                        np.where(g < -1e-12, np.inf, 0.0)))))),
-        gap=float(abs(primal_objective(phi, point_class, classes, w, t, mask) - (-c @ x))),
+        gap=float(abs(primal_objective(phi, point_class, classes, w, t, mask, bot_rows) - (-c @ x))),
     )
     return rep

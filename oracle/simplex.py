@@ -110,8 +110,8 @@ def solve_bounded(c, A, b, u, max_pivots: int = 200000, tol: float = 1e-9):
     return dict(x=x, t=t, opt=float(-c @ x), pivots=it)
 
 
-def solve_plan(phi, point_class, classes, w, mask=None, **kw):
+def solve_plan(phi, point_class, classes, w, mask=None, bot_rows=None, **kw):
     """Exact LP optimum for one plan of a workload."""
     from .lp_model import dual_lp
-    c, A, b, u = dual_lp(phi, point_class, classes, w, mask)
+    c, A, b, u = dual_lp(phi, point_class, classes, w, mask, bot_rows)
     return solve_bounded(c, A, b, u, **kw)

@@ -118,6 +118,8 @@ struct admm_handle {
     float* d_small_t = nullptr;    // [max(N, n)][<= 256] element-major copy of the plan operand of one SpMM
     uint8_t* d_point_class = nullptr;
     double* d_R = nullptr;         // [n]
+    double* d_Rb = nullptr;        // [n] R o bot_rows: b_hat = d_Rb * w_BOT (Eq. 13: only the isocenter rows carry w_BOT with the coupling blocks)
+    double* d_bot = nullptr;       // [n] bot_rows as 0.0 / 1.0
     double* d_Sinv = nullptr;      // [n][lds], lds = n rounded up to even (16-byte rows for cp.async), pad = 0
     int64_t lds = 0;
     int kblk = 32;                 // elements per 128-byte k-block of the stored Phi: 32 (fp32) or 64 (bf16 storage)

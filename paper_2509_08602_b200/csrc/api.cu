@@ -146,7 +146,7 @@ struct Profiler {
 };
 
 void free_all(admm_handle* h) {
-    void* ptrs[] = {h->d_phi, h->d_phiT, h->d_phi_t, h->d_phiT_t, h->d_csr_ptr, h->d_csrT_ptr, h->d_csr_col, h->d_csrT_col, h->d_csr_val, h->d_csrT_val, h->d_small_t, h->d_point_class, h->d_R, h->d_Sinv, h->d_s1, h->d_ghi, h->d_s2, h->d_rhs,
+    void* ptrs[] = {h->d_phi, h->d_phiT, h->d_phi_t, h->d_phiT_t, h->d_csr_ptr, h->d_csrT_ptr, h->d_csr_col, h->d_csrT_col, h->d_csr_val, h->d_csrT_val, h->d_small_t, h->d_point_class, h->d_R, h->d_Rb, h->d_bot, h->d_Sinv, h->d_s1, h->d_ghi, h->d_s2, h->d_rhs,
                     h->d_vhi, h->d_partial, h->d_resid1, h->d_resid2, h->d_hinge, h->d_mask, h->d_slot_plan,
                     h->d_utab, h->d_crtab, h->d_beta, h->d_rho, h->d_active_counts, h->d_conv_flags, h->d_bact, h->d_moves,
                     h->d_nmoves, h->d_iters_plan, h->d_res_plan, h->d_wnorm, h->d_t_f32, h->d_obj, h->d_plan_slot, h->d_tout,
@@ -439,6 +439,16 @@ static admm_status setup_impl(admm_handle* h, const float* phi, int32_t phi_on_d
     h->h_R.resize(n);
     CU_TRY(h, cudaMemcpyAsync(h->h_R.data(), h->d_R, (size_t)n * 8, cudaMemcpyDeviceToHost, st));
     CU_TRY(h, cudaStreamSynchronize(st));
+    {   // b_hat = R o bot_rows * w_BOT (Eq. 13); the option's host pointer is not kept
+        std::vector<double> bot((size_t)n, 1.0), rb((size_t)n);
+        if (h->opt.bot_rows) for (int64_t j = 0; j < n; ++j) bot[j] = h->opt.bot_rows[j] ? 1.0 : 0.0;
+        for (int64_t j = 0; j < n; ++j) rb[j] = h->h_R[j] * bot[j];
+        ST_TRY(dev_alloc(h, &h->d_Rb, n));
+        ST_TRY(dev_alloc(h, &h->d_bot, n));
+        CU_TRY(h, cudaMemcpy(h->d_Rb, rb.data(), (size_t)n * 8, cudaMemcpyHostToDevice));
+        CU_TRY(h, cudaMemcpy(h->d_bot, bot.data(), (size_t)n * 8, cudaMemcpyHostToDevice));
+        h->opt.bot_rows = nullptr;
+    }
     const double t3 = now_ms();
 
     // ---- work decomposition of the two contractions
@@ -485,7 +495,8 @@ admm_status admm_setup(admm_handle** out, const float* phi, int32_t phi_on_devic
     for (int k = 0; k < n_classes; ++k) {
         if (classes[k].sense != 1 && classes[k].sense != -1) { g_setup_err = "class sense must be +1 or -1"; return ADMM_EINVAL; }
         if (!(classes[k].threshold > 0.f) || !std::isfinite(classes[k].threshold)) { g_setup_err = "class threshold must be finite and > 0"; return ADMM_EINVAL; }
-        if (classes[k].hard != 0 && classes[k].hard != 1) { g_setup_err = "class hard must be 0 or 1"; return ADMM_EINVAL; }
+        if (classes[k].hard < 0 || classes[k].hard > 2) { g_setup_err = "class hard must be 0, 1 or 2"; return ADMM_EINVAL; }
+        if (classes[k].hard == 2 && classes[k].threshold != 1.f) { g_setup_err = "a homogeneous hard class (hard = 2) must have threshold 1"; return ADMM_EINVAL; }
     }
     admm_options o;
     if (opt) o = *opt; else admm_default_options(&o);
@@ -493,7 +504,8 @@ admm_status admm_setup(admm_handle** out, const float* phi, int32_t phi_on_devic
     if (!(o.eps_abs > 0.f)) o.eps_abs = 1e-6f;
     if (o.storage < ADMM_STORAGE_FP32_3XTF32 || o.storage > ADMM_STORAGE_CSR) { g_setup_err = "unknown storage mode"; return ADMM_EINVAL; }
     if (o.compaction != 1) { g_setup_err = "compaction must be 1 (masking without compaction is not offered)"; return ADMM_EINVAL; }
-    for (int r : o.reserved) if (r != 0) { g_setup_err = "admm_options.reserved must be 0"; return ADMM_EINVAL; }
+    if (o.bot_rows) for (int64_t j = 0; j < n; ++j)
+        if (o.bot_rows[j] > 1) { g_setup_err = "bot_rows entries must be 0 or 1"; return ADMM_EINVAL; }
     if (o.dose_only != 0 && o.dose_only != 1) { g_setup_err = "dose_only must be 0 or 1"; return ADMM_EINVAL; }
     if (o.dose_only && o.storage == ADMM_STORAGE_CSR) { g_setup_err = "dose_only is not offered with ADMM_STORAGE_CSR"; return ADMM_EINVAL; }
     if (o.storage == ADMM_STORAGE_CSR) {
@@ -665,7 +677,7 @@ admm_status admm_solve_batch(admm_handle* h, int32_t B, const float* weights, co
     int64_t n_min_class = h->class_count[0];
     for (int k = 1; k < K; ++k) n_min_class = std::min(n_min_class, h->class_count[k]);
     bool box_optimum_finite = true;           // presolve needs a finite box optimum: no hard class with c < 0
-    for (int k = 0; k < K; ++k) if (h->classes[k].hard && h->classes[k].sense > 0) box_optimum_finite = false;
+    for (int k = 0; k < K; ++k) if (h->classes[k].hard == 1 && h->classes[k].sense > 0) box_optimum_finite = false;   // c < 0 with u = infinity
     for (int p = 0; p < B; ++p) {
         const double beta = weights[(size_t)p * W + K];
         // default: (kappa / N_min) sqrt(beta0 / max(beta, beta0/floor)), kappa = 1, beta0 = 0.05 (reading R8)
@@ -678,7 +690,7 @@ admm_status admm_solve_batch(admm_handle* h, int32_t B, const float* weights, co
             float uh = (float)(Nkp > 0 ? wk * thr * Nk / Nkp : 0.0);
             if (h->classes[k].hard) uh = Nkp > 0 ? INFINITY : 0.f;
             T.utab[(size_t)k * kMaxBpad + p] = uh;
-            T.crtab[(size_t)k * kMaxBpad + p] = (float)((-sense / Nk) / r);
+            T.crtab[(size_t)k * kMaxBpad + p] = h->classes[k].hard == 2 ? 0.f : (float)((-sense / Nk) / r);   // c = 0 for a homogeneous hard class
             T.wnorm[(size_t)p * kMaxClasses + k] = (Nkp > 0 && !h->classes[k].hard) ? wk / Nkp : 0.0;
         }
         h->slot_plan[p] = p; h->plan_slot[p] = p;

@@ -193,13 +193,13 @@ __global__ void state_out_kernel(const EpiParams ep, int slot, const double* __r
 }
 
 // t = rho R max(s2 - R beta, 0): fp32 output + tf32 hi/lo operand of the objective contraction
-__global__ void make_t_kernel(const double* __restrict__ s2, const double* __restrict__ R, const double* __restrict__ beta,
-                              const double* __restrict__ rho, int64_t n, int64_t ldn, int Bact,
+__global__ void make_t_kernel(const double* __restrict__ s2, const double* __restrict__ R, const double* __restrict__ Rb,
+                              const double* __restrict__ beta, const double* __restrict__ rho, int64_t n, int64_t ldn, int Bact,
                               void* __restrict__ t_hi, void* __restrict__ t_lo, float* __restrict__ t_f32, int bf16) {
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int p = blockIdx.y;
     if (j >= n || p >= Bact) return;
-    double y2 = fmax(s2[(int64_t)p * ldn + j] - R[j] * beta[p], 0.0);
+    double y2 = fmax(s2[(int64_t)p * ldn + j] - Rb[j] * beta[p], 0.0);          // b_hat_j = R_j w_BOT on the rows that carry it (Eq. 13)
     double t = rho[p] * R[j] * y2;
     emit_small(t_hi, t_lo, (int64_t)p * ldn, j, t, bf16 != 0);
     t_f32[(int64_t)p * ldn + j] = (float)t;
@@ -208,9 +208,9 @@ __global__ void make_t_kernel(const double* __restrict__ s2, const double* __res
 // ------------------------------------------------------------------------------------------ K2a: rhs of Eq. (6)
 // rhs[p][j] = R_j * sum_slots partial[slot][p][j - 128 mt]  -  (2 z2 - s2)[p][j]     (fp64)
 __global__ void k2a_kernel(const float* __restrict__ partial, const int32_t* __restrict__ mtile_slot_begin, int n_mma,
-                           const double* __restrict__ s2, const double* __restrict__ R, const double* __restrict__ beta,
-                           int64_t n, int64_t ldn, int slot0, int nact, const int32_t* __restrict__ bact_dev,
-                           double* __restrict__ rhs) {
+                           const double* __restrict__ s2, const double* __restrict__ R, const double* __restrict__ Rb,
+                           const double* __restrict__ beta, int64_t n, int64_t ldn, int slot0, int nact,
+                           const int32_t* __restrict__ bact_dev, double* __restrict__ rhs) {
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int p = blockIdx.y;                       // index inside this contraction pass
     if (bact_dev) nact = min(nact, *bact_dev - slot0);
@@ -221,7 +221,7 @@ __global__ void k2a_kernel(const float* __restrict__ partial, const int32_t* __r
         w += (double)partial[((int64_t)s * n_mma + p) * kTileM + jl];
     const int gs = slot0 + p;
     double sv = s2[(int64_t)gs * ldn + j];
-    double z = fmin(sv, R[j] * beta[gs]);
+    double z = fmin(sv, Rb[j] * beta[gs]);
     rhs[(int64_t)gs * ldn + j] = R[j] * w - (2.0 * z - sv);
 }
 
@@ -256,7 +256,8 @@ __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
 template <int WJ, int RA>
 __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sinv, int64_t lds,
                                                   const double* __restrict__ rhs, double* __restrict__ s2,
-                                                  const double* __restrict__ R, const double* __restrict__ beta,
+                                                  const double* __restrict__ R, const double* __restrict__ Rb,
+                                                  const double* __restrict__ beta,
                                                   int64_t n, int64_t ldn, int Bact, const int32_t* __restrict__ bact_dev,
                                                   void* __restrict__ v_hi, void* __restrict__ v_lo, int bf16,
                                                   double* __restrict__ resid_partial) {
@@ -375,7 +376,7 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
                 for (int a = 0; a < RA; ++a) {
                     const int64_t j = j0 + wj * RW + a * 8 + g;
                     if (j >= n) continue;
-                    const double bh = R[j] * bp;
+                    const double bh = Rb[j] * bp;
                     const double s_old = s2[(int64_t)p * ldn + j];
                     const double z_old = fmin(s_old, bh);
                     const double v = acc[a][b][e];
@@ -518,8 +519,9 @@ __global__ void presolve_state_kernel(const EpiParams ep, int B) {
 }
 // one block per plan
 __global__ void presolve_test_kernel(const float* __restrict__ partial, const int32_t* __restrict__ mtile_slot_begin, int n_mma,
-                                     const double* __restrict__ R, const double* __restrict__ beta, int64_t n, int64_t ldn,
-                                     int slot0, int nact, double margin, double* __restrict__ s2, int32_t* __restrict__ flags) {
+                                     const double* __restrict__ R, const double* __restrict__ Rb, const double* __restrict__ beta,
+                                     int64_t n, int64_t ldn, int slot0, int nact, double margin, double* __restrict__ s2,
+                                     int32_t* __restrict__ flags) {
     const int p = blockIdx.x;
     if (p >= nact) return;
     const int gs = slot0 + p;
@@ -534,7 +536,7 @@ __global__ void presolve_test_kernel(const float* __restrict__ partial, const in
         for (int s = mtile_slot_begin[mt]; s < mtile_slot_begin[mt + 1]; ++s)
             w += (double)partial[((int64_t)s * n_mma + p) * kTileM + jl];
         w *= R[j];
-        if (!(w <= R[j] * bp * (1.0 - margin))) mybad = 1;
+        if (!(w <= Rb[j] * bp * (1.0 - margin))) mybad = 1;
         s2[(int64_t)gs * ldn + j] = w;                     // z2 of the candidate; overwritten with 0 below if it is rejected
     }
     if (mybad) bad = 1;
@@ -656,14 +658,14 @@ __global__ void __launch_bounds__(128) simt_epilogue_kernel(const EpiParams ep, 
 }
 
 
-// obj[slot] = sum_k wnorm[slot][k] * sum_cta hinge[cta][slot][k] + beta[slot] * sum_j t[slot][j]     (fp64)
+// obj[slot] = sum_k wnorm[slot][k] * sum_cta hinge[cta][slot][k] + beta[slot] * sum_j bot[j] t[slot][j]     (fp64)
 __global__ void objective_reduce_kernel(const double* __restrict__ hinge, int grid, const double* __restrict__ wnorm,
-                                        const double* __restrict__ beta, const float* __restrict__ t, int64_t n, int64_t ldn,
-                                        int B, double* __restrict__ obj) {
+                                        const double* __restrict__ beta, const double* __restrict__ bot, const float* __restrict__ t,
+                                        int64_t n, int64_t ldn, int B, double* __restrict__ obj) {
     int p = blockIdx.x;
     if (p >= B) return;
     double acc = 0.0;
-    for (int64_t j = threadIdx.x; j < n; j += blockDim.x) acc += (double)t[(int64_t)p * ldn + j];
+    for (int64_t j = threadIdx.x; j < n; j += blockDim.x) acc += bot[j] * (double)t[(int64_t)p * ldn + j];     // the rows that carry w_BOT
     acc *= beta[p];
     for (int i = threadIdx.x; i < grid * kMaxClasses; i += blockDim.x) {
         int g = i / kMaxClasses, k = i % kMaxClasses;
@@ -775,7 +777,7 @@ void launch_emit_g(const EpiParams& ep, int Bact, cudaStream_t s) {
 }
 void launch_k2a(admm_handle* h, int slot0, int nact, int n_mma, cudaStream_t s) {
     dim3 grid((unsigned)cdiv(h->n, 128), nact);
-    k2a_kernel<<<grid, 128, 0, s>>>(h->d_partial, h->d_mtile_slot_begin, n_mma, h->d_s2, h->d_R, h->d_beta, h->n, h->ldn,
+    k2a_kernel<<<grid, 128, 0, s>>>(h->d_partial, h->d_mtile_slot_begin, n_mma, h->d_s2, h->d_R, h->d_Rb, h->d_beta, h->n, h->ldn,
                                     slot0, nact, h->d_bact, h->d_rhs);
     h->launch_count++;
 }
@@ -804,7 +806,7 @@ static void launch_k2b_t(admm_handle* h, int Bact, bool resid, cudaStream_t s) {
     // the attribute is per device: set it per handle and instantiation (a process-wide flag would leave a second device without the opt-in)
     if (h->k2_attr_tj != TJ) { cudaFuncSetAttribute(k2b_kernel<WJ, RA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); h->k2_attr_tj = TJ; }
     dim3 grid((unsigned)cdiv(h->n, TJ), (unsigned)cdiv(Bact, K2_TP));
-    k2b_kernel<WJ, RA><<<grid, 256, smem, s>>>(h->d_Sinv, h->lds, h->d_rhs, h->d_s2, h->d_R, h->d_beta, h->n, h->ldn, Bact, h->d_bact,
+    k2b_kernel<WJ, RA><<<grid, 256, smem, s>>>(h->d_Sinv, h->lds, h->d_rhs, h->d_s2, h->d_R, h->d_Rb, h->d_beta, h->n, h->ldn, Bact, h->d_bact,
                                                h->d_vhi, h->d_vlo, h->opt.storage == ADMM_STORAGE_BF16 ? 1 : 0,
                                                resid ? h->d_resid2 : nullptr);
 }
@@ -863,7 +865,7 @@ void launch_presolve_state(const EpiParams& ep, int B, cudaStream_t s) {
     presolve_state_kernel<<<grid, 256, 0, s>>>(ep, B);
 }
 void launch_presolve_test(admm_handle* h, int slot0, int nact, int n_mma, double margin, cudaStream_t s) {
-    presolve_test_kernel<<<nact, 256, 0, s>>>(h->d_partial, h->d_mtile_slot_begin, n_mma, h->d_R, h->d_beta, h->n, h->ldn, slot0, nact,
+    presolve_test_kernel<<<nact, 256, 0, s>>>(h->d_partial, h->d_mtile_slot_begin, n_mma, h->d_R, h->d_Rb, h->d_beta, h->n, h->ldn, slot0, nact,
                                                margin, h->d_s2, h->d_conv_flags);
 }
 void launch_presolve_reset(admm_handle* h, int B, cudaStream_t s) {
@@ -875,7 +877,7 @@ void launch_init_plan_records(admm_handle* h, int B, cudaStream_t s) {
 }
 void launch_make_t(admm_handle* h, int Bact, void* t_hi, void* t_lo, float* t_f32, cudaStream_t s) {
     dim3 grid((unsigned)cdiv(h->n, 128), Bact);
-    make_t_kernel<<<grid, 128, 0, s>>>(h->d_s2, h->d_R, h->d_beta, h->d_rho, h->n, h->ldn, Bact, t_hi, t_lo, t_f32,
+    make_t_kernel<<<grid, 128, 0, s>>>(h->d_s2, h->d_R, h->d_Rb, h->d_beta, h->d_rho, h->n, h->ldn, Bact, t_hi, t_lo, t_f32,
                                        h->opt.storage == ADMM_STORAGE_BF16 ? 1 : 0);
     h->launch_count++;
 }
@@ -888,7 +890,7 @@ void launch_reduce_partial(admm_handle* h, int nact, int n_mma, double* out, cud
 }
 void launch_objective_reduce(admm_handle* h, int B, int grid, const float* t_f32, const double* wnorm, double* obj_slot,
                              cudaStream_t s) {
-    objective_reduce_kernel<<<B, 256, 0, s>>>(h->d_hinge, grid, wnorm, h->d_beta, t_f32, h->n, h->ldn, B, obj_slot);
+    objective_reduce_kernel<<<B, 256, 0, s>>>(h->d_hinge, grid, wnorm, h->d_beta, h->d_bot, t_f32, h->n, h->ldn, B, obj_slot);
     h->launch_count++;
 }
 void launch_lowdose_volume(const float* dose, int64_t ld, int64_t N, int B, float lo, float hi, uint32_t* in_vol, int64_t words,
@@ -903,5 +905,5 @@ void launch_gather_rows(const float* src, int64_t ld, const int32_t* plan_slot, 
 void launch_state_out(admm_handle* h, const EpiParams& ep, int slot, float* z1, float* y1, double* z2,
                       double* y2, cudaStream_t s) {
     int64_t m = h->N > h->n ? h->N : h->n;
-    state_out_kernel<<<(unsigned)cdiv(m, 256), 256, 0, s>>>(ep, slot, h->d_s2, h->d_R, h->d_beta, z1, y1, z2, y2);
+    state_out_kernel<<<(unsigned)cdiv(m, 256), 256, 0, s>>>(ep, slot, h->d_s2, h->d_Rb, h->d_beta, z1, y1, z2, y2);     // Rb: the bound b_hat = Rb w_BOT
 }

@@ -24,4 +24,5 @@ from .generate import (  # noqa: F401
     uniform01,
     weight_grid,
     with_plans_of,
+    with_sector_coupling,
 )

@@ -76,6 +76,7 @@ class Workload:
     isocenters: np.ndarray = field(repr=False, default=None)   # [n_iso, 3] mm
     radii: np.ndarray = field(repr=False, default=None)
     centres: np.ndarray = field(repr=False, default=None)
+    bot_rows: Optional[np.ndarray] = field(repr=False, default=None)   # [n] uint8: rows of A that carry w_BOT in b (None = all)
 
     @property
     def N(self) -> int:
@@ -104,7 +105,7 @@ class Workload:
             point_class=self.point_class, classes=self.classes, weights=self.weights[plans].copy(),
             row_mask=None if self.row_mask is None else self.row_mask[plans].copy(),
             alpha=self.alpha[plans].copy(), beta=self.beta[plans].copy(), points=self.points,
-            isocenters=self.isocenters, radii=self.radii, centres=self.centres)
+            isocenters=self.isocenters, radii=self.radii, centres=self.centres, bot_rows=self.bot_rows)
 
 
 # name -> (n_targets, total_volume_mm3, N_T, N_L, shell_outer_mm, n_iso, grid, masked)
@@ -388,3 +389,27 @@ def pick_from_union(union: np.ndarray, count: int, seed: int) -> np.ndarray:
         return idx
     u = uniform01(SEED_BASE + _S_PICK + 1000003 * int(seed), idx.astype(np.uint64))
     return np.sort(idx[np.argsort(u, kind="stable")[:count]])
+
+
+
+def with_sector_coupling(w: Workload, scale: float = 1.0) -> Workload:
+    """The case of `w` with the sector / isocenter coupling of PAPER.md App. A (Eq. 12, 16, 17, :316, :330-332): one time variable
+    tau_iso per isocenter is appended (n -> n + N_iso) and one dual variable per (isocenter, sector) (N -> N + 8 N_iso), whose
+    row of the extended Phi is  -1/scale on the three collimator times of that sector (C = I (x) I_8 (x) 1_{1x3}) and +1 on tau_iso
+    (T = I (x) 1_{8x1}); its class is homogeneous hard (sense +1, threshold 1, hard = 2: c = 0, u = infinity) and only the tau rows
+    carry w_BOT in b (Eq. 13).  Column j of w.phi is time variable (iso*8 + s)*3 + c."""
+    n_iso = w.n // (N_SECTORS * len(COLLIMATOR_SIGMA_MM))
+    assert n_iso * N_SECTORS * len(COLLIMATOR_SIGMA_MM) == w.n and w.row_mask is None
+    n_c = N_SECTORS * n_iso
+    phi = np.zeros((w.N + n_c, w.n + n_iso), dtype=np.float32)
+    phi[:w.N, :w.n] = w.phi
+    for k in range(n_c):
+        phi[w.N + k, 3 * k:3 * k + 3] = -1.0 / scale
+        phi[w.N + k, w.n + k // N_SECTORS] = 1.0
+    pc = np.concatenate([w.point_class, np.full(n_c, len(w.classes), dtype=np.uint8)])
+    classes = list(w.classes) + [ClassSpec(+1, 1.0, hard=2)]
+    weights = np.concatenate([w.weights[:, :-1], np.zeros((w.B, 1)), w.weights[:, -1:]], axis=1)     # the coupling class has no weight
+    bot = np.concatenate([np.zeros(w.n, np.uint8), np.ones(n_iso, np.uint8)])
+    return Workload(name=w.name + "+coupling", config=w.config, phi=phi, point_class=pc, classes=classes, weights=weights,
+                    row_mask=None, alpha=w.alpha, beta=w.beta, points=w.points, isocenters=w.isocenters, radii=w.radii,
+                    centres=w.centres, bot_rows=bot)

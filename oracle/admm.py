@@ -25,6 +25,11 @@ alone is x_box = u where c < 0, 0 where c > 0.  If A x_box <= b it is feasible f
 the multipliers of A x <= b vanish (t* = 0), and Eq. (6), (7), (4b), (4c) have the fixed point
     z1 = x_box,  y1 = -c/rho,  z2 = A x_box,  y2 = 0        (v = 0 in Eq. 6)
 which is returned for such a plan with 0 iterations.
+
+Optional warm start (NOT in the paper; DESIGN.md deviation D3, off by default, with presolve only): a plan whose box optimum is NOT
+feasible but violates A x <= b by at most a factor `warm_start_ratio` in every row ((A x_box)_j <= ratio * b_j) starts from
+    z1 = x_box,  y1 = -c/rho,  z2 = min(A x_box, b),  y2 = A x_box - z2
+instead of the zero iterate (R6).  The iteration itself and its fixed points are unchanged; only the starting point differs.
 """
 from __future__ import annotations
 
@@ -109,9 +114,19 @@ def presolve_box_optimum(pre: Preconditioned, u_hat, b_hat, rho, margin: float =
     return accepted, state
 
 
+def warm_start_plans(accepted, state, b_hat, ratio: float):
+    """Plans that start from the box state (module docstring): rejected by the presolve, finite box optimum, and
+    (A x_box)_j <= ratio * b_j in every row.  Returns (warm [B] bool, z2, y2 of the warm start)."""
+    Ax = state["z2"]
+    finite = np.all(np.isfinite(state["z1"]), axis=0)
+    warm = (~accepted) & finite & np.all(Ax <= ratio * b_hat, axis=0) if ratio > 0 else np.zeros_like(accepted)
+    z2 = np.minimum(Ax, b_hat)
+    return warm, z2, Ax - z2
+
+
 def admm_run(pre: Preconditioned, u_hat, b_hat, rho, iters: int, tol: Optional[float] = None,
              eps_abs: float = 1e-6, check_every: int = 10, state0=None, history: bool = False,
-             presolve: bool = False):
+             presolve: bool = False, warm_start_ratio: float = 0.0):
     """Run `iters` iterations (tol=None) or until every plan meets the stopping rule / iters.
     presolve=True (tolerance mode only): see presolve_box_optimum."""
     A = pre.A_hat
@@ -136,6 +151,10 @@ def admm_run(pre: Preconditioned, u_hat, b_hat, rho, iters: int, tol: Optional[f
             arr[:, presolved] = ps[name][:, presolved]
         active &= ~presolved
         converged |= presolved
+        if warm_start_ratio > 0:
+            warm, wz2, wy2 = warm_start_plans(presolved, ps, b_hat, warm_start_ratio)
+            z1[:, warm] = ps["z1"][:, warm]; y1[:, warm] = ps["y1"][:, warm]
+            z2[:, warm] = wz2[:, warm]; y2[:, warm] = wy2[:, warm]
     for k in range(1, iters + 1):
         r1 = z1 - y1 - c_over_rho
         r2 = z2 - y2
@@ -186,7 +205,8 @@ def recover(pre: Preconditioned, state, rho):
     return t, lam
 
 
-def solve_workload(w, rho, iters, tol=None, check_every=10, eps_abs=1e-6, pre=None, history=False, presolve=False):
+def solve_workload(w, rho, iters, tol=None, check_every=10, eps_abs=1e-6, pre=None, history=False, presolve=False,
+                   warm_start_ratio=0.0):
     """Convenience: precondition + bounds + run + recover + primal objective per plan."""
     from .lp_model import hard_violation, primal_terms
     if pre is None:
@@ -195,7 +215,7 @@ def solve_workload(w, rho, iters, tol=None, check_every=10, eps_abs=1e-6, pre=No
     bot_rows = getattr(w, "bot_rows", None)
     u_hat, b_hat = plan_bounds(pre, w.point_class, w.classes, w.weights, masks, bot_rows)
     st = admm_run(pre, u_hat, b_hat, rho, iters, tol=tol, eps_abs=eps_abs, check_every=check_every,
-                  history=history, presolve=presolve)
+                  history=history, presolve=presolve, warm_start_ratio=warm_start_ratio)
     t, lam = recover(pre, st, rho)
     # obj: the penalty terms of the soft classes + the BOT term at t (a hard class is a constraint, reported as its violation)
     hard = np.array([bool(getattr(c, "hard", 0)) for c in w.classes])

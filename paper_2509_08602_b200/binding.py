@@ -43,7 +43,7 @@ class admm_options(C.Structure):
                 ("check_every", C.c_int32), ("eps_abs", C.c_float), ("compaction", C.c_int32),
                 ("csr_rel_threshold", C.c_float), ("profile_kernels", C.c_int32), ("drain_kb", C.c_int32),
                 ("k1_slab_kb", C.c_int32), ("presolve", C.c_int32), ("accum_debias", C.c_int32), ("dose_only", C.c_int32),
-                ("bot_rows", C.c_void_p)]
+                ("warm_start_ratio", C.c_float), ("bot_rows", C.c_void_p)]
 
 
 def _load() -> C.CDLL:
@@ -124,7 +124,7 @@ def admm_setup(phi, point_class, classes: Sequence, *, storage: int = ADMM_STORA
                check_every: int = 10, eps_abs: float = 1e-6, compaction: bool = True,
                profile_kernels: bool = False, drain_kb: int = 0, k1_slab_kb: int = 0,
                csr_rel_threshold: float = 0.0, presolve: bool = True, accum_debias: int = 0,
-               dose_only: bool = False, bot_rows=None) -> Handle:
+               dose_only: bool = False, bot_rows=None, warm_start_ratio: float = 0.0) -> Handle:
     """phi: [N, n] float32, numpy (host) or torch CUDA tensor, row-major (last stride 1).
     classes: sequence of objects with .sense, .threshold, .hard (e.g. workloads.ClassSpec)."""
     if _is_torch(phi):
@@ -147,6 +147,7 @@ def admm_setup(phi, point_class, classes: Sequence, *, storage: int = ADMM_STORA
     o.presolve = int(presolve)
     o.accum_debias = int(accum_debias)
     o.dose_only = int(dose_only)
+    o.warm_start_ratio = float(warm_start_ratio)
     br = None
     if bot_rows is not None:
         br = np.ascontiguousarray(bot_rows, dtype=np.uint8)

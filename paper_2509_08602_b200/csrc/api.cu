@@ -507,6 +507,8 @@ admm_status admm_setup(admm_handle** out, const float* phi, int32_t phi_on_devic
     if (o.bot_rows) for (int64_t j = 0; j < n; ++j)
         if (o.bot_rows[j] > 1) { g_setup_err = "bot_rows entries must be 0 or 1"; return ADMM_EINVAL; }
     if (o.dose_only != 0 && o.dose_only != 1) { g_setup_err = "dose_only must be 0 or 1"; return ADMM_EINVAL; }
+    if (!(o.warm_start_ratio >= 0.f) || !std::isfinite(o.warm_start_ratio)) { g_setup_err = "warm_start_ratio must be finite and >= 0"; return ADMM_EINVAL; }
+    if (o.warm_start_ratio > 0.f && o.warm_start_ratio < 1.f) { g_setup_err = "warm_start_ratio, if set, must be >= 1"; return ADMM_EINVAL; }
     if (o.dose_only && o.storage == ADMM_STORAGE_CSR) { g_setup_err = "dose_only is not offered with ADMM_STORAGE_CSR"; return ADMM_EINVAL; }
     if (o.storage == ADMM_STORAGE_CSR) {
         // sparse contractions run on the plain FP32 ALUs with the orchestration of the cross-check path

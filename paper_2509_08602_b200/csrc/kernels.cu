@@ -517,41 +517,51 @@ __global__ void presolve_state_kernel(const EpiParams ep, int B) {
     const float ub = mask_ub(ep, cls, p, i);
     ep.s1[(int64_t)p * ep.ldN + i] = (cr < 0.f ? ub : 0.f) - cr;
 }
-// one block per plan
+// one block per plan.  flags: 1 = accepted (settled, 0 iterations); 0 = rejected, starts from the zero iterate (R6); 2 = rejected
+// but warm-started (deviation D3): its box optimum violates A x <= b by at most a factor warm_ratio in every row, and the box
+// state (z1 = x_box, y1 = -c/rho, z2 = min(A x_box, b), y2 = the excess) is kept as its initial iterate.
 __global__ void presolve_test_kernel(const float* __restrict__ partial, const int32_t* __restrict__ mtile_slot_begin, int n_mma,
                                      const double* __restrict__ R, const double* __restrict__ Rb, const double* __restrict__ beta,
-                                     int64_t n, int64_t ldn, int slot0, int nact, double margin, double* __restrict__ s2,
-                                     int32_t* __restrict__ flags) {
+                                     int64_t n, int64_t ldn, int slot0, int nact, double margin, double warm_ratio,
+                                     double* __restrict__ s2, int32_t* __restrict__ flags) {
     const int p = blockIdx.x;
     if (p >= nact) return;
     const int gs = slot0 + p;
-    __shared__ int bad;
-    if (threadIdx.x == 0) bad = 0;
+    __shared__ int bad, cold;
+    if (threadIdx.x == 0) { bad = 0; cold = 0; }
     __syncthreads();
     const double bp = beta[gs];
-    int mybad = 0;
+    int mybad = 0, mycold = 0;
     for (int64_t j = threadIdx.x; j < n; j += blockDim.x) {
         const int mt = (int)(j / kTileM), jl = (int)(j % kTileM);
         double w = 0.0;
         for (int s = mtile_slot_begin[mt]; s < mtile_slot_begin[mt + 1]; ++s)
             w += (double)partial[((int64_t)s * n_mma + p) * kTileM + jl];
         w *= R[j];
-        if (!(w <= Rb[j] * bp * (1.0 - margin))) mybad = 1;
-        s2[(int64_t)gs * ldn + j] = w;                     // z2 of the candidate; overwritten with 0 below if it is rejected
+        const double bj = Rb[j] * bp;
+        if (!(w <= bj * (1.0 - margin))) mybad = 1;
+        if (!(w <= bj * warm_ratio)) mycold = 1;           // (A x_box)_j / b_j above the ratio (or b_j = 0 < (A x_box)_j)
+        s2[(int64_t)gs * ldn + j] = w;                     // s2 = A x_box of the candidate; overwritten with 0 below for a cold start
     }
     if (mybad) bad = 1;
+    if (mycold) cold = 1;
     __syncthreads();
-    const int rejected = bad;
-    if (rejected)
+    const int rejected = bad, warm = rejected && warm_ratio > 0.0 && !cold;
+    if (rejected && !warm)
         for (int64_t j = threadIdx.x; j < n; j += blockDim.x) s2[(int64_t)gs * ldn + j] = 0.0;
-    if (threadIdx.x == 0) flags[gs] = rejected ? 0 : 1;
+    if (threadIdx.x == 0) flags[gs] = rejected ? (warm ? 2 : 0) : 1;
 }
-// zero start (R6) for the plans the presolve did not accept; their K1 operand is re-emitted by emit_g afterwards
+// zero start (R6) for the plans the presolve neither accepted nor warm-started; their K1 operand is re-emitted by emit_g afterwards
 __global__ void presolve_reset_kernel(const int32_t* __restrict__ flags, float* __restrict__ s1, int64_t N, int64_t ldN, int B) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int p = blockIdx.y;
     if (i >= N || p >= B || flags[p]) return;
     s1[(int64_t)p * ldN + i] = 0.f;
+}
+// after the reset: only the accepted plans stay flagged (the compaction freezes every flagged slot)
+__global__ void presolve_flags_kernel(int32_t* __restrict__ flags, int B) {
+    int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < B) flags[p] = flags[p] == 1 ? 1 : 0;
 }
 __global__ void set_iters_kernel(const int32_t* __restrict__ flags, int B, int32_t* __restrict__ iters_plan, float* __restrict__ res_plan) {
     int p = blockIdx.x * blockDim.x + threadIdx.x;        // slot == plan before any compaction
@@ -866,11 +876,12 @@ void launch_presolve_state(const EpiParams& ep, int B, cudaStream_t s) {
 }
 void launch_presolve_test(admm_handle* h, int slot0, int nact, int n_mma, double margin, cudaStream_t s) {
     presolve_test_kernel<<<nact, 256, 0, s>>>(h->d_partial, h->d_mtile_slot_begin, n_mma, h->d_R, h->d_Rb, h->d_beta, h->n, h->ldn, slot0, nact,
-                                               margin, h->d_s2, h->d_conv_flags);
+                                               margin, (double)h->opt.warm_start_ratio, h->d_s2, h->d_conv_flags);
 }
 void launch_presolve_reset(admm_handle* h, int B, cudaStream_t s) {
     dim3 grid((unsigned)cdiv(h->N, 256), B);
     presolve_reset_kernel<<<grid, 256, 0, s>>>(h->d_conv_flags, h->d_s1, h->N, h->ldN, B);
+    presolve_flags_kernel<<<(unsigned)cdiv(B, 128), 128, 0, s>>>(h->d_conv_flags, B);
 }
 void launch_init_plan_records(admm_handle* h, int B, cudaStream_t s) {
     set_iters_kernel<<<(unsigned)cdiv(B, 128), 128, 0, s>>>(h->d_conv_flags, B, h->d_iters_plan, h->d_res_plan);

@@ -33,7 +33,7 @@ def test_option_struct_matches_header(binding):
     assert (o.storage, o.kernel_path, o.check_every, o.compaction) == (0, 0, 10, 1)
     assert abs(o.eps_abs - 1e-6) < 1e-12
     import ctypes
-    assert ctypes.sizeof(binding.admm_options) == 4 * 3 + 4 + 8 + 4 * 5 + 4 * 7     # incl. pointer alignment padding
+    assert ctypes.sizeof(binding.admm_options) == 4 * 3 + 4 + 8 + 4 * 10 + 4 + 4 + 8     # incl. pointer alignment padding (80 bytes)
 
 
 def test_no_cpu_fallback_and_argument_errors(binding):

@@ -406,6 +406,56 @@ def test_converged_objectives_match_simplex_config0(b):
     assert np.array_equal(out["iters"] == 0, ref["presolved"])
 
 
+def test_warm_start_matches_oracle(b):
+    """Deviation D3 (admm_options.warm_start_ratio): the plans the presolve rejects narrowly start from the box state.  Fifty
+    iterations in tolerance mode (tol too small to stop anything) from that start must give the oracle's iterates -- same
+    selection of plans, same starting point, same iteration -- and the untouched plans must be bit-identical to a run without the
+    option.  Then to convergence: same objectives as from the zero start."""
+    from oracle import admm
+    from workloads import Workload, make_workload, scaled_rho
+    w0 = make_workload(2, n_target=1500, n_lowdose=3000, n_iso=18, grid=3)            # 9 targets, row masks
+    pre = admm.precondition(w0.phi, w0.point_class, w0.classes)
+    m1 = w0.mask_bool()[:1]
+    u1, b1 = admm.plan_bounds(pre, w0.point_class, w0.classes, np.array([[1.0, 0.5, 1.0]]), m1)
+    _, st1 = admm.presolve_box_optimum(pre, u1, b1, np.array([1e-3]))
+    beta_star = float(np.max(st1["z2"] / b1))
+    betas = np.tile(beta_star * np.array([1.3, 0.9, 0.6, 0.3, 0.1]), 3)                # ratios ~0.8 (accepted), 1.1, 1.7, 3.3, 10
+    alphas = np.repeat([0.25, 0.5, 1.0], 5)
+    weights = np.stack([np.ones(15), alphas, betas], axis=1)
+    from workloads import pack_mask
+    masks = np.repeat(m1, 15, axis=0)
+    w = Workload(name="warm", config=2, phi=w0.phi, point_class=w0.point_class, classes=w0.classes, weights=weights,
+                 row_mask=pack_mask(masks), alpha=alphas, beta=betas)
+    rho = scaled_rho(betas, w0.point_class)
+    ref = admm.solve_workload(w, rho, 50, tol=1e-12, pre=pre, presolve=True, warm_start_ratio=2.5)
+    u_hat, b_hat = admm.plan_bounds(pre, w.point_class, w.classes, weights, masks)
+    acc, ps = admm.presolve_box_optimum(pre, u_hat, b_hat, rho)
+    warm, _, _ = admm.warm_start_plans(acc, ps, b_hat, 2.5)
+    assert 3 <= warm.sum() <= 9 and acc.sum() >= 3 and (~acc & ~warm).sum() >= 3
+    h = b.admm_setup(w.phi, w.point_class, w.classes, warm_start_ratio=2.5)
+    out = b.admm_solve_batch(h, w.weights, rho, w.row_mask, tol=1e-12, max_iter=50)
+    states = _gpu_states(b, h, w.B)
+    assert np.array_equal(out["iters"] == 0, acc)
+    ez, ey = stacked_errors(states, ref)
+    et = t_errors(out["t"], ref["t"])
+    assert ez.max() < TOL_FP32 and ey.max() < TOL_FP32 and et.max() < 2e-4, (ez, ey, et)
+    hot = b.admm_solve_batch(h, w.weights, rho, w.row_mask, tol=1e-4, max_iter=6000)
+    h.close()
+    h = b.admm_setup(w.phi, w.point_class, w.classes)
+    out0 = b.admm_solve_batch(h, w.weights, rho, w.row_mask, tol=1e-12, max_iter=50)
+    st0 = _gpu_states(b, h, w.B)
+    cold = b.admm_solve_batch(h, w.weights, rho, w.row_mask, tol=1e-4, max_iter=6000)
+    h.close()
+    for p in np.nonzero(~warm)[0]:                                                    # not selected: the option changes nothing
+        assert np.array_equal(out["t"][p], out0["t"][p])
+        for a, c in zip(states[p], st0[p]):
+            assert np.array_equal(a, c)
+    for p in np.nonzero(warm)[0]:                                                     # selected: another start, the same optimum
+        assert not np.array_equal(states[p][0], st0[p][0])
+        if hot["iters"][p] < 6000 and cold["iters"][p] < 6000:
+            assert abs(hot["obj"][p] - cold["obj"][p]) / max(abs(cold["obj"][p]), 0.1) < 1e-3
+
+
 def test_presolve_matches_oracle(b):
     """Deviation D1: plans whose box optimum is feasible are settled before iterating, with the ADMM fixed point as their state
     (oracle/admm.py presolve_box_optimum); the other plans are not touched by the option (bit-identical to presolve off)."""

@@ -96,7 +96,7 @@ typedef struct {
     float   warm_start_ratio;  /* > 0 (with presolve = 1, tolerance mode): a plan the presolve rejects whose box optimum violates A x <= b by at
                                   most this factor in every row ((A x_box)_j <= ratio * b_j) starts from the box state z1 = x_box,
                                   y1 = -c/rho, z2 = min(A x_box, b), y2 = A x_box - z2 instead of the zero iterate (deviation D3; the
-                                  plans next to the presolve threshold: 3x fewer iterations at ratio 2.5).  0 (default): zero start */
+                                  plans next to the presolve threshold of config 3 need 2.4x fewer iterations at ratio 2.5).  0 (default): zero start */
     const uint8_t* bot_rows;   /* HOST [n] 0/1 or NULL: the time variables whose row of A carries w_BOT in b (Eq. 13: b = (0, w_BOT): with
                                   the coupling blocks only the isocenter times do; P(t) then charges w_BOT * sum of THOSE t_j).  NULL =
                                   all n of them (the LP without coupling).  Read during admm_setup only. */

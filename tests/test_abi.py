@@ -51,6 +51,14 @@ def test_no_cpu_fallback_and_argument_errors(binding):
     with pytest.raises(binding.AdmmError) as e:
         binding.admm_setup(w.phi, w.point_class, w.classes, storage=binding.ADMM_STORAGE_BF16, kernel_path=binding.ADMM_PATH_SIMT)
     assert e.value.status == binding.ADMM_EINVAL
+    for kw in (dict(warm_start_ratio=0.5), dict(warm_start_ratio=float("nan")), dict(bot_rows=np.full(w.n, 2, np.uint8))):
+        with pytest.raises(binding.AdmmError) as e:                                            # new options: range checks
+            binding.admm_setup(w.phi, w.point_class, w.classes, **kw)
+        assert e.value.status == binding.ADMM_EINVAL, kw
+    for cls in (dict(sense=1, threshold=1.0, hard=3), dict(sense=1, threshold=0.5, hard=2)):   # hard in {0,1,2}; hard = 2 needs threshold 1
+        with pytest.raises(binding.AdmmError) as e:
+            binding.admm_setup(w.phi, w.point_class, [type("C", (), cls)(), w.classes[1]])
+        assert e.value.status == binding.ADMM_EINVAL, cls
     bad = [type("C", (), dict(sense=2, threshold=1.0, hard=0))(), w.classes[1]]
     with pytest.raises(binding.AdmmError) as e:
         binding.admm_setup(w.phi, w.point_class, bad)

@@ -67,3 +67,23 @@ def test_converged_coupled_objectives_match_the_simplex(b):
         assert abs(out["obj"][p] - soft) / max(abs(soft), 0.1) < 1e-4                 # the library's P(t): w_BOT on the isocenter times only
         checked += 1
     assert checked >= 4
+
+
+def test_fixed_k_parity_with_coupling_multitarget_and_row_masks(b):
+    """The coupled problem on the multi-target geometry with per-plan low-dose row masks (configs 2-4's structure): 9 targets,
+    18 isocenters (n = 432 + 18), 25 plans; K = 50 iterates against the oracle."""
+    from oracle import admm
+    from workloads import make_workload, scaled_rho, with_sector_coupling
+    w0 = make_workload(2, n_target=1500, n_lowdose=3000, n_iso=18, grid=5)
+    w = with_sector_coupling(w0)
+    assert w.row_mask is not None and w.mask_bool()[:, w0.N:].all()
+    rho = 0.3 * scaled_rho(w.beta, w0.point_class)
+    ref = admm.solve_workload(w, rho, 50)
+    h = b.admm_setup(w.phi, w.point_class, w.classes, bot_rows=w.bot_rows)
+    out = b.admm_solve_batch(h, w.weights, rho, w.row_mask, fixed_iters=50)
+    states = [b.admm_get_state(h, p) for p in range(w.B)]
+    h.close()
+    ez, ey = stacked_errors(states, ref)
+    et = t_errors(out["t"], ref["t"])
+    deg = (w.alpha == 0) & (w.beta == 0)
+    assert ez.max() < TOL_FP32 and ey.max() < TOL_FP32 and et[~deg].max() < TOL_FP32, (ez.max(), ey.max(), et)

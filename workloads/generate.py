@@ -399,7 +399,7 @@ def with_sector_coupling(w: Workload, scale: float = 1.0) -> Workload:
     (T = I (x) 1_{8x1}); its class is homogeneous hard (sense +1, threshold 1, hard = 2: c = 0, u = infinity) and only the tau rows
     carry w_BOT in b (Eq. 13).  Column j of w.phi is time variable (iso*8 + s)*3 + c."""
     n_iso = w.n // (N_SECTORS * len(COLLIMATOR_SIGMA_MM))
-    assert n_iso * N_SECTORS * len(COLLIMATOR_SIGMA_MM) == w.n and w.row_mask is None
+    assert n_iso * N_SECTORS * len(COLLIMATOR_SIGMA_MM) == w.n
     n_c = N_SECTORS * n_iso
     phi = np.zeros((w.N + n_c, w.n + n_iso), dtype=np.float32)
     phi[:w.N, :w.n] = w.phi
@@ -410,6 +410,9 @@ def with_sector_coupling(w: Workload, scale: float = 1.0) -> Workload:
     classes = list(w.classes) + [ClassSpec(+1, 1.0, hard=2)]
     weights = np.concatenate([w.weights[:, :-1], np.zeros((w.B, 1)), w.weights[:, -1:]], axis=1)     # the coupling class has no weight
     bot = np.concatenate([np.zeros(w.n, np.uint8), np.ones(n_iso, np.uint8)])
+    row_mask = None
+    if w.row_mask is not None:                        # the coupling variables are active in every plan
+        row_mask = pack_mask(np.concatenate([w.mask_bool(), np.ones((w.B, n_c), dtype=bool)], axis=1))
     return Workload(name=w.name + "+coupling", config=w.config, phi=phi, point_class=pc, classes=classes, weights=weights,
-                    row_mask=None, alpha=w.alpha, beta=w.beta, points=w.points, isocenters=w.isocenters, radii=w.radii,
+                    row_mask=row_mask, alpha=w.alpha, beta=w.beta, points=w.points, isocenters=w.isocenters, radii=w.radii,
                     centres=w.centres, bot_rows=bot)

@@ -47,6 +47,13 @@ def test_dose_matches_the_definition(b, case):
             b.admm_solve_batch(h, np.ones((B, 2)), None, fixed_iters=1)
         assert e.value.status == b.ADMM_ESTATE
         h.close()
+    # the SIMT cross-check path serves the same call
+    t = np.abs(rng.standard_normal((5, w.n))).astype(np.float32) * 0.02
+    h = b.admm_setup(phic, np.zeros(phic.shape[0], np.uint8), w.classes[:1], dose_only=True, kernel_path=b.ADMM_PATH_SIMT)
+    got = b.admm_dose(h, t)
+    h.close()
+    ex = t.astype(np.float64) @ phic.astype(np.float64).T
+    assert np.max(np.abs(got - ex) / (np.abs(t.astype(np.float64)) @ np.abs(phic.astype(np.float64)).T + 1e-30)) < 2e-6
     # bf16 storage: against the rounded matrix the kernels consume, bf16 hi/lo time vectors (2^-17)
     t = np.abs(rng.standard_normal((9, w.n))).astype(np.float32) * 0.02
     Pr = _round_bf16(phic).astype(np.float64)

@@ -87,3 +87,21 @@ def test_fixed_k_parity_with_coupling_multitarget_and_row_masks(b):
     et = t_errors(out["t"], ref["t"])
     deg = (w.alpha == 0) & (w.beta == 0)
     assert ez.max() < TOL_FP32 and ey.max() < TOL_FP32 and et[~deg].max() < TOL_FP32, (ez.max(), ey.max(), et)
+
+
+def test_coupling_with_reduced_storage(b):
+    """The coupling rows (-1 / +1) are exact in tf32 and bf16, so the reduced-storage modes solve the coupled LP of the rounded Phi:
+    K = 50 iterates against the oracle on the ORIGINAL Phi inside north_star's 1e-2 budget."""
+    from oracle import admm
+    from workloads import make_workload, scaled_rho, with_sector_coupling
+    w0 = make_workload(0, n_target=600, n_lowdose=1200, n_iso=4, grid=3)
+    w = with_sector_coupling(w0)
+    rho = 0.3 * scaled_rho(w.beta, w0.point_class)
+    ref = admm.solve_workload(w, rho, 50)
+    for storage in (b.ADMM_STORAGE_FP32_TF32, b.ADMM_STORAGE_BF16):
+        h = b.admm_setup(w.phi, w.point_class, w.classes, bot_rows=w.bot_rows, storage=storage)
+        out = b.admm_solve_batch(h, w.weights, rho, fixed_iters=50)
+        states = [b.admm_get_state(h, p) for p in range(w.B)]
+        h.close()
+        ez, ey = stacked_errors(states, ref)
+        assert ez.max() < 1e-2 and ey.max() < 1e-2, (storage, ez.max(), ey.max())

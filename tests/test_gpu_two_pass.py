@@ -152,3 +152,29 @@ def test_two_pass_with_algorithm1_sampling(b, case):
     for q in np.nonzero(both)[0]:
         P_ref = lp_model.primal_objective(phi2, pc2, w.classes, ws.weights[q], p2["t"][q], masks2[q])
         assert abs(res["pass2"]["obj"][q] - P_ref) / max(abs(P_ref), 0.1) < 1e-3, (q, res["pass2"]["obj"][q], P_ref)
+
+
+def test_dose_argument_handling(b, case):
+    """Strided t (ld_t > n), a single plan, and the documented argument errors."""
+    import torch
+    w, phic = case
+    h = b.admm_setup(phic, np.zeros(phic.shape[0], np.uint8), w.classes[:1], dose_only=True)
+    big = torch.zeros((3, w.n + 40), dtype=torch.float32)
+    big[:, :w.n] = torch.rand((3, w.n)) * 0.02
+    big[:, w.n:] = 7.0                                                             # must not be read
+    view = big[:, :w.n]                                                            # stride(0) = n + 40
+    got = b.admm_dose(h, view)
+    ex = view.numpy().astype(np.float64) @ phic.astype(np.float64).T
+    assert np.max(np.abs(got - ex)) < 1e-5 * max(1.0, np.abs(ex).max())
+    one = b.admm_dose(h, view[1:2].contiguous())
+    assert np.array_equal(one[0], got[1])                                          # a plan's dose does not depend on the batch
+    with pytest.raises(b.AdmmError) as e:
+        b.admm_lowdose_volumes(h, view.numpy().copy(), 0.5, 0.5)                   # empty range
+    assert e.value.status == b.ADMM_EINVAL
+    with pytest.raises(b.AdmmError) as e:
+        b.admm_contract_probe(h, 0, np.zeros((2, phic.shape[0]), np.float32))      # no Phi^T on a dose-only handle
+    assert e.value.status == b.ADMM_ESTATE
+    with pytest.raises(b.AdmmError) as e:
+        b.admm_get_preconditioner(h)
+    assert e.value.status == b.ADMM_ESTATE
+    h.close()

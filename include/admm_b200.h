@@ -193,6 +193,30 @@ admm_status admm_dose(admm_handle* h, int32_t B, const float* t, int64_t ld_t, f
 admm_status admm_lowdose_volumes(admm_handle* h, int32_t B, const float* t, int64_t ld_t, float d_lo, float d_hi,
                                  uint32_t* in_volume, uint32_t* any_volume, float* dose_out);
 
+/*
+ * The dose-rate contraction of Eq. (6) (PAPER.md:89: W = G . Phi, all plans at once, :96) for callers that may not allocate: code
+ * under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc.  No handle, no set-up call, and NO cudaMalloc / cudaFree
+ * / allocating library routine in any call: the split-K partial sums and arrival counters live in one file-scope __device__ array of
+ * ADMM_STATIC_SCRATCH_BYTES that every GPU which loads the library holds until the process exits.  Plain fp32 FFMA accumulation per
+ * split (a variant of the ADMM_PATH_SIMT cross-check kernel, not the tcgen05 path), partial sums added in split order in fp64: the
+ * same call gives the same bits every time.
+ *     w_out[p][j] = sum_i g[p][i] * phi[i][j]
+ *   phi     [N][ld] fp32 row-major, DEVICE pointer (the layout admm_setup takes), ld >= n
+ *   g       [B][ld_g] fp32, DEVICE pointer, ld_g >= N
+ *   w_out   [B][n] fp64, DEVICE pointer, dense
+ *   device  CUDA device ordinal all three pointers belong to;  stream: cudaStream_t the work is enqueued on (NULL = legacy default)
+ *   errbuf  HOST buffer of errbuf_len bytes that receives the message of a failed call (NUL-terminated), or NULL
+ * Limit: B * n <= (ADMM_STATIC_SCRATCH_BYTES - 16384) / 4 = 2093056 outputs (e.g. 218 plans at n = 9600) and at most 4096 output
+ * tiles of 64 x 64; beyond that the call fails with ADMM_EINVAL and touches nothing.  N is not limited.
+ * Asynchronous: returns once the work is enqueued (one memset of the arrival counters, one kernel); it does not synchronise.
+ * The first call on a device resolves the scratch array's address (cudaGetSymbolAddress, which loads the module): make it outside
+ * stream capture.  Every call on a device shares the one array: calls that can overlap on the GPU (different streams, no ordering
+ * between them) RACE on it -- order them.  Host threads may call concurrently as far as the library's own state goes.
+ */
+#define ADMM_STATIC_SCRATCH_BYTES (8 * 1024 * 1024)
+admm_status admm_phit_apply_static(const float* phi, int64_t N, int64_t n, int64_t ld, const float* g, int64_t ld_g, int32_t B,
+                                   double* w_out, int32_t device, void* stream, char* errbuf, int32_t errbuf_len);
+
 /* Copies the preconditioner (fp64, HOST pointers, any may be NULL): D [N], R [n], Sinv [n][n]. */
 admm_status admm_get_preconditioner(admm_handle* h, double* D, double* R, double* Sinv);
 

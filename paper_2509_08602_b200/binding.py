@@ -24,7 +24,7 @@ ADMM_PATH_TCGEN05, ADMM_PATH_SIMT = 0, 1
 EXPORTS = [
     "admm_default_options", "admm_setup", "admm_solve_batch", "admm_get_state", "admm_get_preconditioner",
     "admm_get_timing", "admm_get_kernel_times", "admm_last_launch_count", "admm_last_error", "admm_destroy",
-    "admm_version", "admm_contract_probe", "admm_dose", "admm_lowdose_volumes",
+    "admm_version", "admm_contract_probe", "admm_dose", "admm_lowdose_volumes", "admm_phit_apply_static",
 ]
 
 
@@ -69,6 +69,8 @@ def _load() -> C.CDLL:
     lib.admm_contract_probe.argtypes = [vp, i32, i32, vp, vp]; lib.admm_contract_probe.restype = i32
     lib.admm_dose.argtypes = [vp, i32, vp, i64, vp]; lib.admm_dose.restype = i32
     lib.admm_lowdose_volumes.argtypes = [vp, i32, vp, i64, f32, f32, vp, vp, vp]; lib.admm_lowdose_volumes.restype = i32
+    lib.admm_phit_apply_static.argtypes = [vp, i64, i64, i64, vp, i64, i32, vp, i32, vp, C.c_char_p, i32]
+    lib.admm_phit_apply_static.restype = i32
     return lib
 
 
@@ -225,6 +227,30 @@ def admm_lowdose_volumes(h: Handle, t, d_lo: float, d_hi: float, want_dose: bool
     dose = np.empty((B, h.N), dtype=np.float32) if want_dose else None
     _check(_lib.admm_lowdose_volumes(h.ptr, B, _ptr(t), t.shape[1], float(d_lo), float(d_hi), _ptr(inv), _ptr(anyv), _ptr(dose)), h.ptr)
     return (inv, anyv, dose) if want_dose else (inv, anyv)
+
+
+ADMM_STATIC_SCRATCH_BYTES = 8 * 1024 * 1024
+
+
+def admm_phit_apply_static(phi, g, w_out, *, stream=None) -> None:
+    """w_out [B, n] float64 = g [B, N] . phi [N, n], all three torch CUDA tensors of one device (include/admm_b200.h
+    admm_phit_apply_static): allocates nothing, enqueues on `stream` (a cudaStream_t as int; default: torch's current stream) and
+    does not synchronise.  phi / g: float32, last stride 1; w_out: float64, contiguous.  B * n <= 2093056."""
+    import torch
+    for x, dt in ((phi, torch.float32), (g, torch.float32), (w_out, torch.float64)):
+        assert _is_torch(x) and x.is_cuda and x.dim() == 2 and x.dtype == dt and x.stride(1) == 1
+    N, n = int(phi.shape[0]), int(phi.shape[1])
+    B = int(g.shape[0])
+    assert int(g.shape[1]) == N and tuple(w_out.shape) == (B, n) and w_out.is_contiguous()
+    dev = phi.device.index
+    assert g.device.index == dev and w_out.device.index == dev
+    if stream is None:
+        stream = torch.cuda.current_stream(dev).cuda_stream
+    err = C.create_string_buffer(512)
+    st = _lib.admm_phit_apply_static(phi.data_ptr(), N, n, int(phi.stride(0)), g.data_ptr(), int(g.stride(0)), B, w_out.data_ptr(),
+                                     int(dev), C.c_void_p(stream), err, 512)
+    if st != ADMM_OK:
+        raise AdmmError(st, err.value.decode())
 
 
 def admm_get_preconditioner(h: Handle, want_sinv: bool = True):

@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libadmm_b200.so")
-SOURCES = ["api.cu", "gemm_tc.cu", "kernels.cu", "csr.cu"]
+SOURCES = ["api.cu", "gemm_tc.cu", "kernels.cu", "csr.cu", "no_alloc.cu"]
 HEADERS = ["admm_internal.h", "tc_ptx.cuh", "epilogue.cuh", os.path.join("..", "..", "include", "admm_b200.h")]
 
 

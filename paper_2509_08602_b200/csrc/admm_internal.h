@@ -123,7 +123,7 @@ struct admm_handle {
     double* d_Sinv = nullptr;      // [n][lds], lds = n rounded up to even (16-byte rows for cp.async), pad = 0
     int64_t lds = 0;
     int kblk = 32;                 // elements per 128-byte k-block of the stored Phi: 32 (fp32) or 64 (bf16 storage)
-    int k2_wj = 1;                 // K2b block tile = 16 * k2_wj rows (chosen when the batch buffers are allocated)
+    int k2_rows = 16;              // rows of the K2b block tile: 16 / 32 / 40 / 48 / 64 (k2_choose_rows, when the batch buffers are allocated)
     std::vector<double> h_R;
 
     // per-solve state (reallocated when B grows)
@@ -210,6 +210,6 @@ void launch_lowdose_volume(const float* dose, int64_t ld, int64_t N, int B, floa
 void launch_gather_rows(const float* src, int64_t ld, const int32_t* plan_slot, int B, int64_t n, float* dst, cudaStream_t s);
 void launch_state_out(admm_handle* h, const EpiParams& ep, int slot, float* z1, float* y1, double* z2, double* y2, cudaStream_t s);
 int k2b_grid(const admm_handle* h, int Bact);
-int k2_choose_wj(const admm_handle* h, int Bpad);
+int k2_choose_rows(const admm_handle* h, int Bpad);
 void launch_split_small(const float* x, int64_t count, int64_t ld, void* hi, void* lo, bool bf16, cudaStream_t s);
 void launch_reduce_partial(admm_handle* h, int nact, int n_mma, double* out, cudaStream_t s);

@@ -545,7 +545,7 @@ static admm_status ensure_batch_buffers(admm_handle* h, int B) {
     const bool simt = h->opt.kernel_path == ADMM_PATH_SIMT;
     h->map_cache.clear();
     h->Bpad = 0;
-    h->k2_wj = k2_choose_wj(h, Bpad);
+    h->k2_rows = k2_choose_rows(h, Bpad);
     ST_TRY(dev_alloc(h, &h->d_s1, (int64_t)Bpad * h->ldN));
     ST_TRY(dev_alloc(h, &h->d_ghi, 2 * (int64_t)Bpad * h->ldN));          // hi plane, then lo plane
     h->d_glo = h->d_ghi + (int64_t)Bpad * h->ldN;

@@ -239,7 +239,10 @@ constexpr int K2_TP = 96, K2_KC = 64, K2_LD = K2_KC + 4;       // 64-column chun
 constexpr int K2_TPR = K2_KC / 2, K2_RPP = 256 / K2_TPR;        // loader: threads per row (16-byte pieces), rows per pass
 // ring depth: as many 32-column chunks as fit in ~200 KB (the operands come from L2 / HBM at ~1 us latency and the
 // DMMA work per chunk is a few hundred cycles: bytes in flight are what sets the speed)
-__host__ __device__ constexpr int k2_stages(int TJ) { return (200 * 1024) / ((TJ + K2_TP) * K2_LD * 8) > 8 ? 8 : (200 * 1024) / ((TJ + K2_TP) * K2_LD * 8); }
+#ifndef K2_SMEM_KB
+#define K2_SMEM_KB 200        // (226 gives 32- and 40-row tiles a third stage: measured 4 % slower at 32 rows, 0-3 % faster at 40)
+#endif
+__host__ __device__ constexpr int k2_stages(int TJ) { return (K2_SMEM_KB * 1024) / ((TJ + K2_TP) * K2_LD * 8) > 8 ? 8 : (K2_SMEM_KB * 1024) / ((TJ + K2_TP) * K2_LD * 8); }
 
 __device__ __forceinline__ void cp_async16_zfill(void* smem_dst, const void* gsrc, bool ok) {
     const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
@@ -275,7 +278,12 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
     const int64_t j0 = (int64_t)blockIdx.x * TJ;
     const int p0 = blockIdx.y * K2_TP;
     const int nchunks = (int)((n + K2_KC - 1) / K2_KC);
-    const bool warp_live = p0 + wp * 48 < Bact;
+    // the 12 plan fragments of 8 are dealt to the two plan halves alternately (wp = 0: fragments 0, 2, ..; wp = 1: 1, 3, ..), so that a
+    // partly filled tile leaves both halves -- they sit on different SM sub-partitions, each with its own DMMA pipe -- the same work:
+    // nb = this warp's live fragments.  Which warp computes a plan does not change the order its dot products are summed in.
+    const int nfrag = min(12, (Bact - p0 + 7) >> 3);
+    const int nb = (nfrag - wp + 1) >> 1;
+    const bool warp_live = nb > 0;
 
     // loader: thread t copies 16-byte pieces (row = t/16 + 16 i, columns kk, kk+1) for i < NCP; pointers are set up once
     constexpr int NCP = ROWS * (K2_KC / 2) / NT;             // 14 / 16 / 20 for WJ = 1 / 2 / 4 (exact)
@@ -317,7 +325,7 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
         cp_async_commit();
         if (warp_live) {
             const double* sA = k2sm + (size_t)(c % K2_STAGES) * ROWS * K2_LD + (wj * RW + g) * K2_LD + q;
-            const double* sB = k2sm + (size_t)(c % K2_STAGES) * ROWS * K2_LD + (TJ + wp * 48 + g) * K2_LD + q;
+            const double* sB = k2sm + (size_t)(c % K2_STAGES) * ROWS * K2_LD + (TJ + wp * 8 + g) * K2_LD + q;
 #pragma unroll
             for (int i = 0; i < K2_KC / 4 / KS; ++i) {
                 const int ks = kq + i * KS;
@@ -326,9 +334,11 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
                 for (int a = 0; a < RA; ++a) av[a] = sA[a * 8 * K2_LD + ks * 4];
 #pragma unroll
                 for (int b = 0; b < 6; ++b) {
-                    const double bv = sB[b * 8 * K2_LD + ks * 4];
+                    if (b < nb) {
+                        const double bv = sB[b * 16 * K2_LD + ks * 4];
 #pragma unroll
-                    for (int a = 0; a < RA; ++a) dmma884(acc[a][b], av[a], bv);
+                        for (int a = 0; a < RA; ++a) dmma884(acc[a][b], av[a], bv);
+                    }
                 }
             }
         }
@@ -339,7 +349,8 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
     // ---- sum the k-slices in a fixed order: slices 1.. park their fragments, slice 0 adds them
     constexpr int FR = RA * 12;                            // accumulator doubles per thread
     double* red = k2sm;                                    // [(KS-1)][2 WJ warps][FR][32]
-    double* sacc = k2sm + (size_t)3 * 2 * 48 * 32;         // [2 WJ warps][48 plans][kNumResid]  (past the largest red area)
+    constexpr size_t RED = (size_t)(KS - 1) * 2 * WJ * FR * 32;
+    double* sacc = k2sm + (RED > (size_t)3 * 2 * 48 * 32 ? RED : (size_t)3 * 2 * 48 * 32);         // [2 WJ warps][48 plans][kNumResid]  (past the red area)
     if (KS > 1) {
         if (kq > 0) {
             double* dst = red + ((size_t)((kq - 1) * 2 * WJ + wp * WJ + wj) * FR) * 32 + lane;
@@ -361,14 +372,14 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
     }
     const int ew = wp * WJ + wj;                           // index of this (kq == 0) warp among the 2 WJ epilogue warps
 
-    // ---- epilogue-2: thread owns rows j = j0 + wj*RW + a*8 + g, plans p = p0 + wp*48 + b*8 + 2q + e
+    // ---- epilogue-2: thread owns rows j = j0 + wj*RW + a*8 + g, plans p = p0 + (2b + wp)*8 + 2q + e
     const bool resid = resid_partial != nullptr;
     if (kq == 0) {
 #pragma unroll
     for (int b = 0; b < 6; ++b) {
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
-            const int p = p0 + wp * 48 + b * 8 + 2 * q + e;
+            const int p = p0 + (2 * b + wp) * 8 + 2 * q + e;
             double ra[kNumResid] = {0, 0, 0, 0, 0};
             if (p < Bact) {
                 const double bp = beta[p];
@@ -410,10 +421,11 @@ __global__ void __launch_bounds__(256) k2b_kernel(const double* __restrict__ Sin
     if (resid) {
         __syncthreads();
         for (int i = tid; i < K2_TP * kNumResid; i += NT) {
-            const int pp = i / kNumResid, t = i % kNumResid;     // pp in [0, 96): wp = pp / 48
+            const int pp = i / kNumResid, t = i % kNumResid;     // pp in [0, 96): fragment pp / 8 = 2 b + wp
             if (p0 + pp >= Bact) continue;
+            const int f = pp >> 3;
             double v = 0.0;
-            for (int w = 0; w < WJ; ++w) v += sacc[(((pp / 48) * WJ + w) * 48 + pp % 48) * kNumResid + t];
+            for (int w = 0; w < WJ; ++w) v += sacc[((((f & 1) * WJ + w) * 48) + (f >> 1) * 8 + (pp & 7)) * kNumResid + t];
             resid_partial[((int64_t)blockIdx.x * kMaxBpad + p0 + pp) * kNumResid + t] = v;
         }
     }
@@ -791,24 +803,26 @@ void launch_k2a(admm_handle* h, int slot0, int nact, int n_mma, cudaStream_t s) 
                                     slot0, nact, h->d_bact, h->d_rhs);
     h->launch_count++;
 }
-// Rows of the K2b block tile: 64, 32 or 16 (WJ = 4, 2, 1).  One block per SM fits (its cp.async ring takes ~200 KB), so the
-// launch runs in waves of sm_count blocks and the last, partly filled wave costs a full one: n = 9600 is 150 tiles of 64 rows =
-// 2 waves for 148 SMs.  Measured on B200 (n = 9600, <= 96 plans): 1201 / 1019 / 1133 us for 64 / 32 / 16 rows = 2, 3 and 5 waves of
-// blocks that take 1 : 0.57 : 0.38 of a 64-row block's time.  The choice minimises waves x that cost for one tile of plans and depends
-// on n ONLY: the summation order of a row's dot product depends on WJ (4 / WJ k-slices), and a plan must come out bit-identical
-// whatever the batch it is solved in.  (With 441 live plans 64 rows would be 4 % faster than 32 at n = 9600; after the presolve
-// the live count is normally below 96.)
-int k2_choose_wj(const admm_handle* h, int) {
-    const double cost[3] = {0.38, 0.57, 1.0};                   // WJ = 1, 2, 4
-    int best = 1; double best_t = 1e300;
-    for (int i = 0, wj = 1; i < 3; ++i, wj <<= 1) {
-        const double t = (double)cdiv(cdiv(h->n, 16 * wj), h->sm_count) * cost[i];
-        if (t < best_t * (1.0 - 1e-9) || (t <= best_t * (1.0 + 1e-9) && wj > best)) { best_t = std::min(t, best_t); best = wj; }
+// Rows of the K2b block tile: 16, 32, 40, 48 or 64.  One block per SM fits (its cp.async ring takes ~140-200 KB), so the launch runs
+// in waves of sm_count blocks and the last, partly filled wave costs a full one: n = 9600 is 300 tiles of 32 rows = 3 waves for 148
+// SMs, but 240 tiles of 40 rows = 2.  Measured on B200 (96 plans; microseconds per wave per 9600 columns): 215 / 338 / 438 / 511 / 597
+// for 16 / 32 / 40 / 48 / 64 rows = the relative block costs below; K2a + K2b at n = 9600: 1073 / 1015 / 876 / 1022 / 1194 us, at
+// n = 12000: 1586 / 1260 / 1592 / 1244 / 1485 us.  The choice minimises waves x cost and depends on n ONLY: the summation order of a
+// row's dot product depends on the tile (its k-slices), and a plan must come out bit-identical whatever the batch it is solved in.
+int k2_choose_rows(const admm_handle* h, int) {
+#ifdef K2_FORCE_ROWS          // compile-time override, for measuring one tile against another (nvcc -DK2_FORCE_ROWS=32)
+    return K2_FORCE_ROWS;
+#endif
+    const int rows[5] = {16, 32, 40, 48, 64};
+    const double cost[5] = {0.36, 0.57, 0.72, 0.84, 1.0};
+    int best = 16; double best_t = 1e300;
+    for (int i = 0; i < 5; ++i) {
+        const double t = (double)cdiv(cdiv(h->n, rows[i]), h->sm_count) * cost[i];
+        if (t <= best_t * (1.0 + 1e-9)) { best_t = std::min(t, best_t); best = rows[i]; }      // ties go to the larger tile
     }
     return best;
 }
-static int k2_wj(const admm_handle* h) { return h->k2_wj; }
-int k2b_grid(const admm_handle* h, int) { return (int)cdiv(h->n, 16 * k2_wj(h)); }
+int k2b_grid(const admm_handle* h, int) { return (int)cdiv(h->n, h->k2_rows); }
 template <int WJ, int RA>
 static void launch_k2b_t(admm_handle* h, int Bact, bool resid, cudaStream_t s) {
     constexpr int TJ = 8 * RA * WJ;
@@ -821,9 +835,11 @@ static void launch_k2b_t(admm_handle* h, int Bact, bool resid, cudaStream_t s) {
                                                resid ? h->d_resid2 : nullptr);
 }
 void launch_k2b(admm_handle* h, int Bact, bool resid, cudaStream_t s) {
-    switch (k2_wj(h)) {                       // block tile of 64 / 32 / 16 rows
-        case 4: launch_k2b_t<4, 2>(h, Bact, resid, s); break;      // (a 32 x 48 warp tile, <2, 4>, measured slower: 1.42 vs 1.33 ms at config 2)
-        case 2: launch_k2b_t<2, 2>(h, Bact, resid, s); break;
+    switch (h->k2_rows) {                     // <row groups WJ, 8-row fragments per warp RA>: block tile = 8 RA WJ rows
+        case 64: launch_k2b_t<4, 2>(h, Bact, resid, s); break;      // (a 32 x 48 warp tile, <2, 4>, measured slower: 1.42 vs 1.33 ms at config 2)
+        case 48: launch_k2b_t<1, 6>(h, Bact, resid, s); break;
+        case 40: launch_k2b_t<1, 5>(h, Bact, resid, s); break;
+        case 32: launch_k2b_t<2, 2>(h, Bact, resid, s); break;
         default: launch_k2b_t<1, 2>(h, Bact, resid, s); break;
     }
     h->launch_count++;

@@ -67,7 +67,9 @@ enum {
 /* Which kernels run the two Phi contractions. */
 enum {
     ADMM_PATH_TCGEN05 = 0,        /* tcgen05/TMEM/TMA kernels (the product path) */
-    ADMM_PATH_SIMT    = 1         /* plain fp32 FFMA kernels: a slow on-device cross-check, same ABI */
+    ADMM_PATH_SIMT    = 1         /* plain fp32 FFMA kernels: a slow on-device cross-check, same ABI.  They add the K terms of a product
+                                     one after the other in fp32, so their error grows with N: 1e-4 iterate parity holds at the small sizes
+                                     the tests use, not at n ~ 5000, N ~ 15000 (f5) */
 };
 
 typedef struct {
